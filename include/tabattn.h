@@ -1,0 +1,115 @@
+/* libtabattn -- B200 (sm_100a) dual-axis attention for TabPFN-v2-style pretraining.
+ *
+ * The per-layer hot path of the nanoTabPFN pretraining step the paper speedruns
+ * (Fig. 3: every transformer block applies "feature-axis attention,
+ * norm, sample-axis attention, norm, MLP, norm"; both are
+ * explicit-QKV scaled dot-product attention; thinking rows "count as
+ * part of the train portion"; rows are queries, columns are keys).
+ *
+ * Cell tensor layout: every Q/K/V/O/dO/dQ/dK/dV is
+ *     [B tables][R rows][C columns][H heads][dh]      bf16, row-major, dh fastest,
+ * contiguous, 16-byte aligned, d = H*dh.  bf16 crosses this ABI as raw 16-bit
+ * patterns behind void*.  ALL pointers are DEVICE pointers unless a name ends in
+ * _host.  The caller owns every buffer; the library allocates no device memory,
+ * never synchronises the host, and enqueues all work on `stream` (graph-capturable).
+ * Outputs are fully overwritten; inputs are never written; no aliasing of an output
+ * with any other argument.
+ *
+ * Feature attention (a1/a2 of SURVEY.md §8(a)): for each (b, r, h) the sequence runs
+ *   over the table's VALID columns:  S = scale * Q K^T (Cv x Cv), P = softmax_rows(S),
+ *   O = P V, LSE = logsumexp_rows(S) (natural log).            n_train is ignored.
+ * Item attention (a3-a5): for each valid (b, c), each h, every query row i in [0,R)
+ *   attends to key rows j in [0, n_train[b]) only -- train and test queries alike.
+ * Backward (both): D_i = sum_j P_ij dP_ij, dP = dO V^T, dS = P o (dP - D),
+ *   dV = P^T dO, dQ = scale * dS K, dK = scale * dS^T Q; P is recomputed from LSE.
+ *
+ * Masked positions: O, dQ, dK, dV at invalid columns and item dK, dV at rows
+ * >= n_train[b] are written as +0; LSE at invalid columns is 0.0f.  Values stored at
+ * invalid columns of any input, and item K/V at rows >= n_train[b], never influence
+ * an output (even NaN/Inf).  Inputs at valid positions must be finite.
+ */
+#ifndef TABATTN_H_
+#define TABATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TABATTN_VERSION 100   /* major*10000 + minor*100 + patch */
+
+#if defined(__GNUC__)
+#define TABATTN_API __attribute__((visibility("default")))
+#else
+#define TABATTN_API
+#endif
+
+typedef enum {
+  TABATTN_OK = 0,
+  TABATTN_ERR_INVALID_ARG = 1, /* NULL required pointer, non-positive size, misaligned pointer,
+                                  n_train_host[b] outside [1,R], NULL shape */
+  TABATTN_ERR_UNSUPPORTED = 2, /* dh not in {16,32,64}, C > TABATTN_MAX_FEATURE_C for feature_*,
+                                  tensor larger than 2^31 cells, device is not sm_100 */
+  TABATTN_ERR_WORKSPACE = 3,   /* ws == NULL or ws_bytes < tabattn_workspace_bytes(shape, op) */
+  TABATTN_ERR_CUDA = 4         /* a CUDA launch / driver call failed (see cudaGetLastError) */
+} tabattn_status;
+
+/* op codes for tabattn_workspace_bytes */
+enum { TABATTN_OP_FEATURE_FWD = 0, TABATTN_OP_FEATURE_BWD = 1, TABATTN_OP_ITEM_FWD = 2, TABATTN_OP_ITEM_BWD = 3 };
+
+#define TABATTN_MAX_FEATURE_C 128 /* largest column count the feature kernels accept */
+
+typedef struct {
+  int32_t B, R, C, H, dh;       /* all >= 1; dh in {16, 32, 64}                                    */
+  const int32_t* n_train;       /* DEVICE [B]; 1 <= n_train[b] <= R.  item_* only; feature_* ignore
+                                   it (may be NULL there).  Out-of-range device values with no host
+                                   copy are clamped to [1,R] (no device->host error path).          */
+  const int32_t* n_train_host;  /* optional HOST copy [B] (NULL ok): enables the range check         */
+  const uint8_t* col_valid;     /* DEVICE [B*C], nonzero = valid column; NULL = all valid            */
+  float softmax_scale;          /* <= 0.0f  =>  1/sqrt(dh)                                           */
+} tabattn_shape;
+
+/* CUDA stream handle (cudaStream_t) passed as an opaque pointer so that this header needs no
+ * CUDA include; NULL is the legacy default stream. */
+typedef void* tabattn_stream;
+
+/* Feature attention forward.  Q,K,V in; O [B,R,C,H,dh] bf16 and LSE [B,R,H,C] f32 out.
+ * ws/ws_bytes: scratch of at least tabattn_workspace_bytes(shape, TABATTN_OP_FEATURE_FWD)
+ * bytes (may be NULL when that is 0). */
+TABATTN_API tabattn_status tabattn_feature_fwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
+                                   void* O, float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream);
+
+/* Feature attention backward.  O and LSE are the forward's outputs.  dQ,dK,dV out. */
+TABATTN_API tabattn_status tabattn_feature_bwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
+                                   const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
+                                   void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);
+
+/* Item attention forward.  LSE is [B,C,H,R] f32 (contiguous along the sequence). */
+TABATTN_API tabattn_status tabattn_item_fwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
+                                void* O, float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream);
+
+/* Item attention backward: a dQ pass (also emits D = rowsum(dO o O) into the workspace) and a
+ * separate dK/dV pass; deterministic, no atomics. */
+TABATTN_API tabattn_status tabattn_item_bwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
+                                const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
+                                void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);
+
+/* Bytes of device scratch `op` needs for `shape` (0 if shape is NULL or invalid). */
+TABATTN_API size_t tabattn_workspace_bytes(const tabattn_shape* shape, int op);
+
+/* Static, never-NULL description of a status code. */
+TABATTN_API const char* tabattn_status_string(tabattn_status status);
+
+/* Number of CUDA kernels this library has launched in this process so far (all threads, all
+ * streams; monotonically increasing).  Lets a harness count the launches of a timed region. */
+TABATTN_API uint64_t tabattn_launch_count(void);
+
+/* TABATTN_VERSION the library was built with. */
+TABATTN_API int tabattn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TABATTN_H_ */

@@ -1,0 +1,64 @@
+"""One layer of the hot path = the four C-ABI calls of SURVEY.md §8(a), in training order:
+feature fwd, item fwd, item bwd, feature bwd (each block applies feature-axis
+attention then sample-axis attention; backward runs in reverse order).
+
+Marshalling only: buffers are preallocated once (``LayerBuffers``) so the timed region holds
+nothing but kernel launches; ``layer_fwd_bwd_host`` is the same step driven from pinned HOST
+buffers (host->device copies of the eight inputs, device->host read of the results).
+"""
+import torch
+
+from . import binding as _b
+
+
+class LayerBuffers:
+    """Outputs + workspace for one layer of shape [B,R,C,H,dh]; reusable across calls."""
+
+    def __init__(self, B, R, C, H, dh, device="cuda"):
+        shp = (B, R, C, H, dh)
+        bf = dict(dtype=torch.bfloat16, device=device)
+        self.shape = shp
+        self.O_f = torch.empty(shp, **bf)
+        self.O_i = torch.empty(shp, **bf)
+        self.LSE_f = torch.empty((B, R, H, C), dtype=torch.float32, device=device)
+        self.LSE_i = torch.empty((B, C, H, R), dtype=torch.float32, device=device)
+        self.grads_f = tuple(torch.empty(shp, **bf) for _ in range(3))
+        self.grads_i = tuple(torch.empty(shp, **bf) for _ in range(3))
+        probe = torch.empty((0,), **bf)
+        s = _b.TabattnShape(B, R, C, H, dh, None, None, None, 0.0)
+        need = max(_b.workspace_bytes(s, op) for op in range(4))
+        self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
+        del probe
+
+
+def layer_fwd_bwd(feat, item, n_train, col_valid, buf: LayerBuffers, n_train_host=None, stream=None):
+    """Enqueue feature fwd, item fwd, item bwd, feature bwd on the current stream.
+
+    ``feat`` / ``item`` are dicts with device tensors Q, K, V, dO.  Results land in ``buf``."""
+    _b.tabattn_feature_fwd(feat["Q"], feat["K"], feat["V"], col_valid, O=buf.O_f, LSE=buf.LSE_f, ws=buf.ws,
+                           stream=stream)
+    _b.tabattn_item_fwd(item["Q"], item["K"], item["V"], n_train, col_valid, n_train_host=n_train_host,
+                        O=buf.O_i, LSE=buf.LSE_i, ws=buf.ws, stream=stream)
+    _b.tabattn_item_bwd(item["Q"], item["K"], item["V"], buf.O_i, item["dO"], buf.LSE_i, n_train, col_valid,
+                        n_train_host=n_train_host, dQ=buf.grads_i[0], dK=buf.grads_i[1], dV=buf.grads_i[2],
+                        ws=buf.ws, stream=stream)
+    _b.tabattn_feature_bwd(feat["Q"], feat["K"], feat["V"], buf.O_f, feat["dO"], buf.LSE_f, col_valid,
+                           dQ=buf.grads_f[0], dK=buf.grads_f[1], dV=buf.grads_f[2], ws=buf.ws, stream=stream)
+    return buf
+
+
+def layer_fwd_bwd_host(feat_host, item_host, feat_dev, item_dev, out_host, n_train, col_valid,
+                       buf: LayerBuffers, n_train_host=None):
+    """The same step from pinned host buffers: H2D of the 8 inputs, the four calls, D2H of the
+    8 results (O and dQ/dK/dV of both axes) into ``out_host``.  Returns (h2d_bytes, d2h_bytes)."""
+    h2d = d2h = 0
+    for src, dst in ((feat_host, feat_dev), (item_host, item_dev)):
+        for k in ("Q", "K", "V", "dO"):
+            dst[k].copy_(src[k], non_blocking=True)
+            h2d += src[k].numel() * src[k].element_size()
+    layer_fwd_bwd(feat_dev, item_dev, n_train, col_valid, buf, n_train_host)
+    results = (buf.O_f, buf.O_i) + buf.grads_f + buf.grads_i
+    for dst, src in zip(out_host, results):
+        dst.copy_(src, non_blocking=True)
+        d2h += src.numel() * src.element_size()
+    return h2d, d2h

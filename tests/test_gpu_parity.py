@@ -1,0 +1,154 @@
+"""GPU-vs-oracle parity through the C ABI (SURVEY.md §4 tiers T1-T3).  Needs a B200."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from workloads import (get_config, fig6_shape, draw_structure, make_call_inputs, TabShape,  # noqa: E402
+                       f32_to_bf16_bits)
+
+
+def _gu():
+    import gpu_util
+    return gpu_util
+
+
+def _run_case(cfg, axis, n_train=None, col_valid=None, poison=False, what=None):
+    gu = _gu()
+    nt_draw, cv_draw = draw_structure(cfg)
+    n_train = nt_draw if n_train is None else np.asarray(n_train, np.int32)
+    col_valid = cv_draw if col_valid is None else col_valid
+    inp = make_call_inputs(cfg, axis)
+    orc = gu.run_oracle(axis, inp, n_train, col_valid)
+    if poison:
+        # NaN at every position that must not influence any output (SURVEY.md §8(b) "Values at masked positions")
+        nan = np.uint16(0x7FC0)
+        inp = {k: v.copy() for k, v in inp.items()}
+        if col_valid is not None:
+            bad = ~np.asarray(col_valid).astype(bool)
+            for k in ("Q", "K", "V", "dO"):
+                inp[k][np.broadcast_to(bad[:, None, :], inp[k].shape[:3])] = nan
+        if axis == "item":
+            for b in range(cfg.B):
+                inp["K"][b, n_train[b]:] = nan
+                inp["V"][b, n_train[b]:] = nan
+    gpu = gu.run_gpu(axis, inp, n_train, col_valid)
+    return gu.check_parity(axis, inp, gpu, orc, n_train, col_valid, what or "%s/%s" % (cfg.name, axis))
+
+
+# ---- T1: full tensors on the small shapes --------------------------------------------------------
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_tiny_config(axis):
+    _run_case(get_config("tiny"), axis)
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_fig6_shape(axis):
+    # 16 thinking + 80 train + 20 test rows; non-multiple-of-anything
+    _run_case(fig6_shape(), axis)
+
+
+EDGE = [
+    # name, B, R, C, H, dh, n_train
+    ("one_key", 2, 33, 3, 2, 32, 1),          # single key: O = V_0
+    ("no_test_rows", 1, 130, 2, 1, 64, 130),  # n_train = R: plain self-attention, ragged q/k tiles
+    ("one_row", 3, 1, 5, 2, 16, 1),
+    ("one_col", 2, 70, 1, 3, 32, 40),         # feature attention over a single column
+    ("tile_edges", 1, 257, 4, 2, 32, 129),    # one past the 128/256 tile boundaries
+    ("tile_exact", 1, 256, 3, 2, 64, 128),
+    ("wide_C", 1, 9, 128, 1, 32, 5),          # largest feature-axis length
+    ("c17", 2, 40, 17, 2, 32, 30),
+    ("c33_dh64", 1, 24, 33, 2, 64, 17),
+]
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+@pytest.mark.parametrize("case", EDGE, ids=[e[0] for e in EDGE])
+def test_edge_shapes(case, axis):
+    name, B, R, C, H, dh, n = case
+    cfg = TabShape(name, 100 + EDGE.index(case), B=B, R=R, C=C, H=H, dh=dh, n_train=n)
+    _run_case(cfg, axis)
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_ragged_n_train_and_masks_with_nan_poison(axis):
+    cfg = TabShape("mini_ragged", 41, B=4, R=300, C=13, H=2, dh=32, n_train=100, mask="prefix",
+                   ragged_n_train=(1, 300), valid_features=(1, 12))
+    _run_case(cfg, axis, poison=True)
+    cfg = TabShape("mini_subset", 42, B=3, R=150, C=37, H=2, dh=32, n_train=97, mask="subset",
+                   valid_features=(3, 36), q_scale=4.0)
+    _run_case(cfg, axis, poison=True)
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_table_with_no_valid_column(axis):
+    cfg = TabShape("dead_table", 43, B=2, R=64, C=5, H=2, dh=32, n_train=40)
+    cv = np.ones((2, 5), np.uint8)
+    cv[1, :] = 0
+    _run_case(cfg, axis, col_valid=cv, poison=True)
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_all_valid_mask_equals_null_mask(axis):
+    gu = _gu()
+    cfg = TabShape("allvalid", 44, B=2, R=96, C=7, H=2, dh=32, n_train=50)
+    nt, _ = draw_structure(cfg)
+    inp = make_call_inputs(cfg, axis)
+    a = gu.run_gpu(axis, inp, nt, None)
+    b = gu.run_gpu(axis, inp, nt, np.ones((2, 7), np.uint8))
+    for k in ("O", "dQ", "dK", "dV"):
+        assert np.array_equal(gu.to_bits(a[k]), gu.to_bits(b[k]))
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+def test_run_to_run_bitwise_determinism(axis):
+    gu = _gu()
+    cfg = get_config("base").scaled(B=2, R=512, n_train=300)
+    nt, cv = draw_structure(cfg)
+    inp = make_call_inputs(cfg, axis)
+    a = gu.run_gpu(axis, inp, nt, cv)
+    b = gu.run_gpu(axis, inp, nt, cv)
+    for k in ("O", "dQ", "dK", "dV"):
+        assert np.array_equal(gu.to_bits(a[k]), gu.to_bits(b[k])), k
+    assert np.array_equal(a["LSE"].cpu().numpy(), b["LSE"].cpu().numpy())
+
+
+def test_zero_dO_on_train_rows_item():
+    # only test-row outputs feed the loss -> dO = 0 on train rows at the last layer
+    gu = _gu()
+    cfg = TabShape("dO_test_only", 45, B=2, R=200, C=4, H=2, dh=32, n_train=150)
+    nt, cv = draw_structure(cfg)
+    inp = make_call_inputs(cfg, "item")
+    inp["dO"][:, :150] = 0
+    orc = gu.run_oracle("item", inp, nt, cv)
+    gpu = gu.run_gpu("item", inp, nt, cv)
+    gu.check_parity("item", inp, gpu, orc, nt, cv, "dO_test_only")
+    assert gu.is_pos_zero(gu.to_bits(gpu["dQ"])[:, :150] & np.uint16(0x7FFF))
+
+
+def test_custom_softmax_scale():
+    gu = _gu()
+    cfg = TabShape("scale", 46, B=1, R=80, C=6, H=2, dh=32, n_train=60)
+    nt, cv = draw_structure(cfg)
+    for axis in ("feature", "item"):
+        inp = make_call_inputs(cfg, axis)
+        orc = gu.run_oracle(axis, inp, nt, cv, scale=0.31)
+        gpu = gu.run_gpu(axis, inp, nt, cv, scale=0.31)
+        gu.check_parity(axis, inp, gpu, orc, nt, cv, "scale/" + axis)
+
+
+# ---- T2: scaled-down copies of the big configs (several tiles + ragged tails), full tensors -------
+SCALED = [
+    ("base", dict(B=2, R=384, n_train=288)),
+    ("feature_heavy", dict(B=2, R=40, n_train=30)),
+    ("long_item", dict(B=1, R=640, C=3, n_train=480)),
+    ("ragged", dict(B=3, R=400, ragged_n_train=(100, 300))),
+]
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+@pytest.mark.parametrize("name,kw", SCALED, ids=[s[0] for s in SCALED])
+def test_scaled_configs(name, kw, axis):
+    _run_case(get_config(name).scaled(**kw), axis, poison=True)
