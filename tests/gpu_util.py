@@ -72,7 +72,9 @@ def check_parity(axis, inp, gpu, orc, n_train=None, col_valid=None, what=""):
     over valid positions; masked positions bit-exact +0; LSE within LSE_TOL."""
     shape5 = inp["Q"].shape
     cell, key = valid_mask_cells(shape5, axis, n_train, col_valid)
-    vmax = np.abs(bf16_bits_to_f64(inp["V"])).max()
+    # max|V| over the positions that can influence an output (masked V may be NaN-poisoned)
+    v_abs = np.abs(bf16_bits_to_f64(inp["V"]))[key]
+    vmax = v_abs.max() if v_abs.size else 0.0
     out = {}
     for name, mask in (("O", cell), ("dQ", cell), ("dK", key), ("dV", key)):
         bits = to_bits(gpu[name])
