@@ -18,6 +18,7 @@ cudaError_t launch_item_bwd_simt(const Shape& s, const void* Q, const void* K, c
                                  cudaStream_t stream);
 // item_tc_fwd.cu / item_tc_bwd.cu
 bool item_tc_supported(const Shape& s);
+bool item_tc_bwd_supported(const Shape& s);
 cudaError_t launch_item_fwd_tc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                cudaStream_t stream);
 cudaError_t launch_item_bwd_tc(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
@@ -48,7 +49,7 @@ cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const 
                             const void* dO, const float* LSE, void* dQ, void* dK, void* dV, void* ws,
                             cudaStream_t stream) {
   float* Dws = static_cast<float*>(ws);
-  if (!force_simt() && item_tc_supported(s))
+  if (!force_simt() && item_tc_bwd_supported(s))
     return launch_item_bwd_tc(s, Q, K, V, O, dO, LSE, dQ, dK, dV, Dws, stream);
   return launch_item_bwd_simt(s, Q, K, V, O, dO, LSE, dQ, dK, dV, Dws, stream);
 }

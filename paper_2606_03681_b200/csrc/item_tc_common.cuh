@@ -1,0 +1,110 @@
+// Shared pieces of the tcgen05 item-axis kernels (item_tc_fwd.cu, item_tc_bwd.cu): the persistent
+// work walker, the shared-memory tail zeroing that enforces the train-only key rule on partially
+// filled tiles, and the UMMA issue helpers for the two contraction shapes the path needs.
+#pragma once
+#include "common.cuh"
+#include "tc_common.cuh"
+
+namespace tabattn {
+namespace itc {
+
+constexpr int kTileRows = 128;       // rows of every operand tile (UMMA M, and N of the score tiles)
+constexpr float kRescaleLog2 = 8.f;  // lazy-rescale threshold of the online softmax (log2 units)
+
+__device__ __forceinline__ int clamp_n(const Shape& s, int b) { return max(1, min(__ldg(s.n_train + b), s.R)); }
+
+// One CTA walks the work items w = blockIdx.x, blockIdx.x + gridDim.x, ...; an item is one
+// (table b, column c, head h, block of `rows_per_item` rows).  Consecutive items of one (b,c,h) are
+// adjacent in w, so CTAs that run at the same time share K/V (or Q/dO) tiles in L2.  Items of
+// invalid columns are skipped here (the zero-fill of their outputs is done by the epilogue warps).
+// `tiles` = number of 128-row tiles of the looped axis; `t` counts tiles over the CTA's lifetime
+// and `k` counts valid items: they index the mbarrier ring phases.
+struct Walker {
+  int w, j, tiles, n, b, c, h, blk;
+  uint32_t k, t;
+  bool ok;
+
+  __device__ __forceinline__ void decode(const Shape& s, int blocks_per_seq, bool& valid) {
+    blk = w % blocks_per_seq;
+    const int rest = w / blocks_per_seq;
+    h = rest % s.H;
+    const int bc = rest / s.H;
+    b = bc / s.C;
+    c = bc - b * s.C;
+    valid = !s.col_valid || __ldg(s.col_valid + bc) != 0;
+    n = clamp_n(s, b);
+  }
+  // loop_over_keys: the inner axis is the key axis [0, n) (fwd, dQ); otherwise the query axis [0, R)
+  __device__ __forceinline__ void seek(const Shape& s, int n_items, int blocks_per_seq, bool loop_over_keys) {
+    ok = false;
+    while (w < n_items) {
+      bool valid;
+      decode(s, blocks_per_seq, valid);
+      if (valid && (loop_over_keys || blk * kTileRows < n)) {
+        tiles = ((loop_over_keys ? n : s.R) + kTileRows - 1) / kTileRows;
+        j = 0;
+        ok = true;
+        return;
+      }
+      w += gridDim.x;
+    }
+  }
+  __device__ __forceinline__ void init(const Shape& s, int n_items, int bps, bool lk) {
+    w = blockIdx.x; k = 0; t = 0;
+    seek(s, n_items, bps, lk);
+  }
+  __device__ __forceinline__ void next(const Shape& s, int n_items, int bps, bool lk) {
+    ++t;
+    if (++j == tiles) {
+      w += gridDim.x;
+      ++k;
+      seek(s, n_items, bps, lk);
+    }
+  }
+};
+
+// Zero rows [first_row, 128) of a [128][ROWB bytes] tile (whole rows: the 16-byte-chunk swizzle only
+// permutes bytes inside a row).  Called by one full warp after the TMA load has landed; makes the
+// generic-proxy stores visible to the tensor core (async proxy) before returning.
+template <int ROWB>
+__device__ __forceinline__ void zero_tail_rows(uint32_t tile_saddr, int first_row, int lane) {
+  const uint32_t begin = tile_saddr + first_row * ROWB, end = tile_saddr + kTileRows * ROWB;
+  for (uint32_t a = begin + 16 * lane; a < end; a += 16 * 32)
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+  tc::fence_proxy_async_smem();
+  __syncwarp();
+}
+
+// D[128 x 128] (tmem) = A[128 x DH] * B[128 x DH]^T, both K-major tiles as TMA wrote them.
+template <int DH>
+__device__ __forceinline__ void issue_qk(uint32_t d_tmem, uint32_t a_saddr, uint32_t b_saddr) {
+  constexpr int ROWB = DH * 2;
+  constexpr uint32_t idesc = tc::make_idesc_bf16(128, 128, false, false);
+#pragma unroll
+  for (int k = 0; k < DH / 16; ++k)
+    tc::mma_ss(d_tmem, tc::make_smem_desc<ROWB>(a_saddr + 32 * k, 16, 8 * ROWB),
+               tc::make_smem_desc<ROWB>(b_saddr + 32 * k, 16, 8 * ROWB), idesc, k > 0);
+}
+
+// D[128 x DH] (tmem) (+)= A[128 x 128] (bf16 in tmem, 64 columns) * B[128 x DH] (MN-major smem tile).
+template <int DH>
+__device__ __forceinline__ void issue_pv(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_saddr, bool accumulate) {
+  constexpr int ROWB = DH * 2;
+  constexpr uint32_t idesc = tc::make_idesc_bf16(128, DH, false, true);
+#pragma unroll
+  for (int kk = 0; kk < 8; ++kk)
+    tc::mma_ts(d_tmem, a_tmem + 8 * kk, tc::make_smem_desc<ROWB>(b_saddr + kk * 16 * ROWB, 16, 8 * ROWB), idesc,
+               (accumulate || kk > 0) ? 1u : 0u);
+}
+
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() {
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
+}
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() {
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
+}
+
+}  // namespace itc
+}  // namespace tabattn

@@ -1,0 +1,326 @@
+// Item-axis attention forward on tcgen05.
+//
+// Persistent, warp-specialised kernel; one CTA per SM walks work items (b, c, h, 256 query rows):
+//   warp 8        TMA producer: Q tiles (2 x 128 rows, double-buffered over items) and a ring of K/V
+//                 tiles of the train rows [0, n_train[b]) only
+//   warp 9        MMA issuer: S_t = Q_t K_j^T (SS, fp32 in TMEM), O_t += P_t V_j (A = P in TMEM as bf16)
+//   warps 0-3/4-7 softmax warpgroup of query tile t = 0 / 1: one thread per query row reads its S row
+//                 from TMEM, online softmax in base 2 with lazy rescaling of O, writes P (bf16) back
+//                 to TMEM; epilogue O / l -> bf16, LSE (natural log)
+// S for the next key tile is issued before the PV of the current one, across item boundaries, so
+// the softmax warps (the exp-bound critical path at dh <= 64) never wait for the tensor core.
+// Keys >= n_train[b] never reach an output: their S columns are masked to -inf and their K/V rows
+// are zeroed in shared memory after the TMA load.
+#include <cuda.h>
+
+#include <algorithm>
+
+#include "item_tc_common.cuh"
+#include "kernels.h"
+
+namespace tabattn {
+
+namespace {
+
+using namespace tc;
+using namespace itc;
+
+template <int DH>
+struct FwdCfg {
+  static constexpr int ROWB = DH * 2;
+  static constexpr int TILE = kTileRows * ROWB;  // bytes of one 128-row operand tile
+  static constexpr int ST = 3;                   // K/V ring depth
+  static constexpr int QBUF = 2;                 // Q double buffer (over items), 2 tiles each
+  static constexpr int SMEM = (2 * QBUF + 2 * ST) * TILE + 1024;
+  // TMEM columns
+  static constexpr int S0 = 0, P0 = 256, O0 = 384, COLS = 512;
+  static_assert(O0 + 2 * DH <= COLS, "TMEM budget");
+};
+
+constexpr int kFwdThreads = 384;
+
+template <int DH>
+__global__ void __launch_bounds__(kFwdThreads, 1)
+item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
+                   const __grid_constant__ CUtensorMap mapV, Shape s, __nv_bfloat16* __restrict__ O,
+                   float* __restrict__ LSE, int n_items, int blocks_per_seq) {
+  using Cfg = FwdCfg<DH>;
+  constexpr int ST = Cfg::ST, TILE = Cfg::TILE, ROWB = Cfg::ROWB;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = sbase;                               // [QBUF][2][TILE]
+  const uint32_t sK = sQ + 2 * Cfg::QBUF * TILE;           // [ST][TILE]
+  const uint32_t sV = sK + ST * TILE;                      // [ST][TILE]
+  __shared__ uint64_t bar_q_full[2], bar_q_empty[2], bar_k_full[ST], bar_v_full[ST], bar_kv_empty[ST];
+  __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_pv_done[2];
+  __shared__ uint32_t tmem_slot;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (warp == 10) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&bar_q_full[i]), 1);
+      mbar_init(smem_u32(&bar_q_empty[i]), 1);
+      mbar_init(smem_u32(&bar_s_full[i]), 1);
+      mbar_init(smem_u32(&bar_s_empty[i]), 128);
+      mbar_init(smem_u32(&bar_p_full[i]), 128);
+      mbar_init(smem_u32(&bar_pv_done[i]), 1);
+    }
+    for (int i = 0; i < ST; ++i) {
+      mbar_init(smem_u32(&bar_k_full[i]), 1);
+      mbar_init(smem_u32(&bar_v_full[i]), 1);
+      mbar_init(smem_u32(&bar_kv_empty[i]), 1);
+    }
+    fence_barrier_init();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  if (warp >= 8) {
+    setmaxnreg_dec<56>();
+    if (warp == 8) {
+      // ------------------------------------------------------------------ TMA producer
+      if (lane == 0) {
+        tma_prefetch_desc(&mapQ);
+        tma_prefetch_desc(&mapK);
+        tma_prefetch_desc(&mapV);
+        Walker wk;
+        for (wk.init(s, n_items, blocks_per_seq, true); wk.ok; wk.next(s, n_items, blocks_per_seq, true)) {
+          if (wk.j == 0) {
+            const int qb = wk.k & 1;
+            mbar_wait(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
+            mbar_arrive_expect_tx(smem_u32(&bar_q_full[qb]), 2 * TILE);
+            const int q0 = wk.blk * 2 * kTileRows;
+            tma_load_5d(sQ + (2 * qb) * TILE, &mapQ, smem_u32(&bar_q_full[qb]), 0, wk.h, wk.c, q0, wk.b);
+            tma_load_5d(sQ + (2 * qb + 1) * TILE, &mapQ, smem_u32(&bar_q_full[qb]), 0, wk.h, wk.c, q0 + kTileRows,
+                        wk.b);
+          }
+          const int st = wk.t % ST;
+          mbar_wait(smem_u32(&bar_kv_empty[st]), ((wk.t / ST) & 1) ^ 1);
+          mbar_arrive_expect_tx(smem_u32(&bar_k_full[st]), TILE);
+          tma_load_5d(sK + st * TILE, &mapK, smem_u32(&bar_k_full[st]), 0, wk.h, wk.c, wk.j * kTileRows, wk.b);
+          mbar_arrive_expect_tx(smem_u32(&bar_v_full[st]), TILE);
+          tma_load_5d(sV + st * TILE, &mapV, smem_u32(&bar_v_full[st]), 0, wk.h, wk.c, wk.j * kTileRows, wk.b);
+        }
+      }
+    } else if (warp == 9) {
+      // ------------------------------------------------------------------ MMA issuer
+      Walker a, p;  // a: S issue (one tile ahead), p: PV issue
+      a.init(s, n_items, blocks_per_seq, true);
+      p = a;
+      auto issue_s = [&]() {
+        const int qb = a.k & 1, st = a.t % ST;
+        if (a.j == 0) mbar_wait(smem_u32(&bar_q_full[qb]), (a.k >> 1) & 1);
+        mbar_wait(smem_u32(&bar_k_full[st]), (a.t / ST) & 1);
+        const int rem = a.n - a.j * kTileRows;
+        if (rem < kTileRows) zero_tail_rows<ROWB>(sK + st * TILE, rem, lane);
+        if (lane == 0) {
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            mbar_wait(smem_u32(&bar_s_empty[t]), (a.t & 1) ^ 1);
+            tc_fence_after();
+            issue_qk<DH>(tmem + Cfg::S0 + 128 * t, sQ + (2 * qb + t) * TILE, sK + st * TILE);
+            tc_commit(smem_u32(&bar_s_full[t]));
+          }
+          if (a.j == a.tiles - 1) tc_commit(smem_u32(&bar_q_empty[qb]));
+        }
+        __syncwarp();
+        a.next(s, n_items, blocks_per_seq, true);
+      };
+      auto issue_o = [&]() {
+        const int st = p.t % ST;
+        mbar_wait(smem_u32(&bar_v_full[st]), (p.t / ST) & 1);
+        const int rem = p.n - p.j * kTileRows;
+        if (rem < kTileRows) zero_tail_rows<ROWB>(sV + st * TILE, rem, lane);
+        if (lane == 0) {
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            mbar_wait(smem_u32(&bar_p_full[t]), p.t & 1);
+            tc_fence_after();
+            issue_pv<DH>(tmem + Cfg::O0 + DH * t, tmem + Cfg::P0 + 64 * t, sV + st * TILE, p.j > 0);
+            tc_commit(smem_u32(&bar_pv_done[t]));
+          }
+          tc_commit(smem_u32(&bar_kv_empty[st]));
+        }
+        __syncwarp();
+        p.next(s, n_items, blocks_per_seq, true);
+      };
+      if (a.ok) issue_s();
+      while (p.ok) {
+        if (a.ok) issue_s();
+        issue_o();
+      }
+    }
+  } else {
+    // -------------------------------------------------------------------- softmax warpgroups
+    setmaxnreg_inc<224>();
+    const int t = warp >> 2;                  // query tile of this warpgroup
+    const int r = threadIdx.x & 127;          // row inside the tile = TMEM lane
+    const uint32_t lane_base = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
+    const uint32_t tS = lane_base + Cfg::S0 + 128 * t, tP = lane_base + Cfg::P0 + 64 * t,
+                   tO = lane_base + Cfg::O0 + DH * t;
+    const uint32_t b_s_full = smem_u32(&bar_s_full[t]), b_s_empty = smem_u32(&bar_s_empty[t]),
+                   b_p_full = smem_u32(&bar_p_full[t]), b_pv_done = smem_u32(&bar_pv_done[t]);
+    const float c2 = s.scale * kLog2e;
+    const int d = s.H * DH;
+    uint32_t g = 0;  // tiles processed by this CTA so far
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      Walker it;
+      it.w = w;
+      bool valid;
+      it.decode(s, blocks_per_seq, valid);
+      const int row = it.blk * 2 * kTileRows + t * kTileRows + r;
+      __nv_bfloat16* orow = O + (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
+      float* lse = LSE + (((size_t)it.b * s.C + it.c) * s.H + it.h) * s.R + row;
+      if (!valid) {
+        if (row < s.R) {
+#pragma unroll
+          for (int k = 0; k < DH / 8; ++k) stg_v4(orow + 8 * k, make_uint4(0, 0, 0, 0));
+          *lse = 0.f;
+        }
+        continue;
+      }
+      const int tiles = (it.n + kTileRows - 1) / kTileRows;
+      float m = -INFINITY, l = 0.f;
+      for (int j = 0; j < tiles; ++j, ++g) {
+        mbar_wait(b_s_full, g & 1);
+        tc_fence_after();
+        uint32_t sr[128];
+        tmem_ld32(tS, sr);
+        tmem_ld32(tS + 32, sr + 32);
+        tmem_ld32(tS + 64, sr + 64);
+        tmem_ld32(tS + 96, sr + 96);
+        tmem_wait_ld();
+        tc_fence_before();
+        mbar_arrive(b_s_empty);
+        float* sf = reinterpret_cast<float*>(sr);
+        const int rem = it.n - j * kTileRows;
+        if (rem < kTileRows) {
+#pragma unroll
+          for (int k = 0; k < 128; ++k)
+            if (k >= rem) sf[k] = -INFINITY;
+        }
+        float mx0 = sf[0], mx1 = sf[1], mx2 = sf[2], mx3 = sf[3];
+#pragma unroll
+        for (int k = 4; k < 128; k += 4) {
+          mx0 = fmaxf(mx0, sf[k]);
+          mx1 = fmaxf(mx1, sf[k + 1]);
+          mx2 = fmaxf(mx2, sf[k + 2]);
+          mx3 = fmaxf(mx3, sf[k + 3]);
+        }
+        const float mxs = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c2;
+        if (j == 0) {
+          m = mxs;
+        } else if (__any_sync(0xffffffffu, mxs > m + kRescaleLog2)) {
+          // rare after the first tiles: bring the accumulated O and l to the new reference maximum
+          const float mn = fmaxf(m, mxs);
+          const float alpha = fast_exp2(m - mn);
+          l *= alpha;
+          m = mn;
+          mbar_wait(b_pv_done, (g - 1) & 1);
+          tc_fence_after();
+          uint32_t o[DH];
+          tmem_ld_cols<DH>(tO, o);
+#pragma unroll
+          for (int k = 0; k < DH; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
+          tmem_st_cols<DH>(tO, o);
+          tmem_wait_st();
+        }
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        uint32_t p[64];
+#pragma unroll
+        for (int k = 0; k < 64; k += 2) {
+          const float e0 = fast_exp2(fmaf(sf[2 * k], c2, -m));
+          const float e1 = fast_exp2(fmaf(sf[2 * k + 1], c2, -m));
+          const float e2 = fast_exp2(fmaf(sf[2 * k + 2], c2, -m));
+          const float e3 = fast_exp2(fmaf(sf[2 * k + 3], c2, -m));
+          l0 += e0; l1 += e1; l2 += e2; l3 += e3;
+          p[k] = pack_bf16(e0, e1);
+          p[k + 1] = pack_bf16(e2, e3);
+        }
+        l += (l0 + l1) + (l2 + l3);
+        if (g > 0) mbar_wait(b_pv_done, (g - 1) & 1);  // previous PV has finished reading the P buffer
+        tmem_st32(tP, p);
+        tmem_st32(tP + 32, p + 32);
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(b_p_full);
+      }
+      // ---- epilogue: O = acc / l, LSE = ln(sum exp) ---------------------------------------------
+      mbar_wait(b_pv_done, (g - 1) & 1);
+      tc_fence_after();
+      uint32_t o[DH];
+      tmem_ld_cols<DH>(tO, o);
+      tc_fence_before();
+      if (row < s.R) {
+        const float inv = 1.f / l;
+#pragma unroll
+        for (int k = 0; k < DH / 8; ++k) {
+          float f[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(o[8 * k + e]) * inv;
+          stg_v4(orow + 8 * k, pack8(f));
+        }
+        *lse = (m + log2f(l)) * kLn2;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 10) tmem_dealloc(tmem, Cfg::COLS);
+}
+
+template <int DH>
+cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
+                       cudaStream_t stream) {
+  using Cfg = FwdCfg<DH>;
+  CUtensorMap mq, mk, mv;
+  if (!make_cell_tensor_map(&mq, Q, s.B, s.R, s.C, s.H, DH, kTileRows) ||
+      !make_cell_tensor_map(&mk, K, s.B, s.R, s.C, s.H, DH, kTileRows) ||
+      !make_cell_tensor_map(&mv, V, s.B, s.R, s.C, s.H, DH, kTileRows))
+    return cudaErrorInvalidValue;
+  auto kern = item_fwd_tc_kernel<DH>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int bps = (s.R + 2 * kTileRows - 1) / (2 * kTileRows);
+  const long long n_items = (long long)s.B * s.C * s.H * bps;
+  const int grid = (int)std::min<long long>(n_items, num_sms());
+  kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, (int)n_items, bps);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+int num_sms() {
+  static int n = []() {
+    int dev = 0, v = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    return v > 0 ? v : 148;
+  }();
+  return n;
+}
+
+bool item_tc_supported(const Shape& s) {
+  // the tensor-map path needs 16-byte aligned global strides (always true: dh >= 16 bf16) and fits
+  // every shape the ABI accepts; tiny problems also run here (one code path to validate)
+  return s.dh == 16 || s.dh == 32 || s.dh == 64;
+}
+
+cudaError_t launch_item_fwd_tc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
+                               cudaStream_t stream) {
+  switch (s.dh) {
+    case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, stream);
+    case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, stream);
+    case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, stream);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace tabattn

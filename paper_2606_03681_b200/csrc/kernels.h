@@ -24,6 +24,7 @@ cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const 
                             const void* dO, const float* LSE, void* dQ, void* dK, void* dV, void* ws,
                             cudaStream_t stream);
 size_t item_fwd_workspace_bytes(const Shape& s);
+int num_sms();  // SM count of the current device (cached)
 size_t item_bwd_workspace_bytes(const Shape& s);
 
 }  // namespace tabattn
