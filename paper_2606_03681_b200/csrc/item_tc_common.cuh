@@ -23,25 +23,26 @@ struct Walker {
   int w, j, tiles, n, b, c, h, blk;
   uint32_t k, t;
   bool ok;
+  int n_items, bps, chunk;   // items in the launch, 128/256-row blocks per sequence, rows per inner tile
+  bool over_keys;            // inner axis = key rows [0, n) (fwd, dQ); else query rows [0, R) (dK/dV)
 
-  __device__ __forceinline__ void decode(const Shape& s, int blocks_per_seq, bool& valid) {
-    blk = w % blocks_per_seq;
-    const int rest = w / blocks_per_seq;
+  __device__ __forceinline__ void decode(const Shape& s, bool& valid) {
+    blk = w % bps;
+    const int rest = w / bps;
     h = rest % s.H;
     const int bc = rest / s.H;
     b = bc / s.C;
     c = bc - b * s.C;
-    valid = !s.col_valid || __ldg(s.col_valid + bc) != 0;
     n = clamp_n(s, b);
+    valid = (!s.col_valid || __ldg(s.col_valid + bc) != 0) && (over_keys || blk * kTileRows < n);
+    tiles = ((over_keys ? n : s.R) + chunk - 1) / chunk;
   }
-  // loop_over_keys: the inner axis is the key axis [0, n) (fwd, dQ); otherwise the query axis [0, R)
-  __device__ __forceinline__ void seek(const Shape& s, int n_items, int blocks_per_seq, bool loop_over_keys) {
+  __device__ __forceinline__ void seek(const Shape& s) {
     ok = false;
     while (w < n_items) {
       bool valid;
-      decode(s, blocks_per_seq, valid);
-      if (valid && (loop_over_keys || blk * kTileRows < n)) {
-        tiles = ((loop_over_keys ? n : s.R) + kTileRows - 1) / kTileRows;
+      decode(s, valid);
+      if (valid) {
         j = 0;
         ok = true;
         return;
@@ -49,50 +50,51 @@ struct Walker {
       w += gridDim.x;
     }
   }
-  __device__ __forceinline__ void init(const Shape& s, int n_items, int bps, bool lk) {
+  __device__ __forceinline__ void init(const Shape& s, int n_items_, int bps_, int chunk_, bool over_keys_) {
+    n_items = n_items_; bps = bps_; chunk = chunk_; over_keys = over_keys_;
     w = blockIdx.x; k = 0; t = 0;
-    seek(s, n_items, bps, lk);
+    seek(s);
   }
-  __device__ __forceinline__ void next(const Shape& s, int n_items, int bps, bool lk) {
+  __device__ __forceinline__ void next(const Shape& s) {
     ++t;
     if (++j == tiles) {
       w += gridDim.x;
       ++k;
-      seek(s, n_items, bps, lk);
+      seek(s);
     }
   }
 };
 
-// Zero rows [first_row, 128) of a [128][ROWB bytes] tile (whole rows: the 16-byte-chunk swizzle only
+// Zero rows [first_row, ROWS) of a [ROWS][ROWB bytes] tile (whole rows: the 16-byte-chunk swizzle only
 // permutes bytes inside a row).  Called by one full warp after the TMA load has landed; makes the
 // generic-proxy stores visible to the tensor core (async proxy) before returning.
-template <int ROWB>
+template <int ROWB, int ROWS = kTileRows>
 __device__ __forceinline__ void zero_tail_rows(uint32_t tile_saddr, int first_row, int lane) {
-  const uint32_t begin = tile_saddr + first_row * ROWB, end = tile_saddr + kTileRows * ROWB;
+  const uint32_t begin = tile_saddr + first_row * ROWB, end = tile_saddr + ROWS * ROWB;
   for (uint32_t a = begin + 16 * lane; a < end; a += 16 * 32)
     asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
   tc::fence_proxy_async_smem();
   __syncwarp();
 }
 
-// D[128 x 128] (tmem) = A[128 x DH] * B[128 x DH]^T, both K-major tiles as TMA wrote them.
-template <int DH>
+// D[128 x N] (tmem) = A[128 x DH] * B[N x DH]^T, both K-major tiles as TMA wrote them.
+template <int DH, int N = 128>
 __device__ __forceinline__ void issue_qk(uint32_t d_tmem, uint32_t a_saddr, uint32_t b_saddr) {
   constexpr int ROWB = DH * 2;
-  constexpr uint32_t idesc = tc::make_idesc_bf16(128, 128, false, false);
+  constexpr uint32_t idesc = tc::make_idesc_bf16(128, N, false, false);
 #pragma unroll
   for (int k = 0; k < DH / 16; ++k)
     tc::mma_ss(d_tmem, tc::make_smem_desc<ROWB>(a_saddr + 32 * k, 16, 8 * ROWB),
                tc::make_smem_desc<ROWB>(b_saddr + 32 * k, 16, 8 * ROWB), idesc, k > 0);
 }
 
-// D[128 x DH] (tmem) (+)= A[128 x 128] (bf16 in tmem, 64 columns) * B[128 x DH] (MN-major smem tile).
-template <int DH>
+// D[128 x DH] (tmem) (+)= A[128 x KR] (bf16 in tmem, KR/2 columns) * B[KR x DH] (MN-major smem tile).
+template <int DH, int KR = 128>
 __device__ __forceinline__ void issue_pv(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_saddr, bool accumulate) {
   constexpr int ROWB = DH * 2;
   constexpr uint32_t idesc = tc::make_idesc_bf16(128, DH, false, true);
 #pragma unroll
-  for (int kk = 0; kk < 8; ++kk)
+  for (int kk = 0; kk < KR / 16; ++kk)
     tc::mma_ts(d_tmem, a_tmem + 8 * kk, tc::make_smem_desc<ROWB>(b_saddr + kk * 16 * ROWB, 16, 8 * ROWB), idesc,
                (accumulate || kk > 0) ? 1u : 0u);
 }

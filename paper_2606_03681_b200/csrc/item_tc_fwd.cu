@@ -87,7 +87,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         tma_prefetch_desc(&mapK);
         tma_prefetch_desc(&mapV);
         Walker wk;
-        for (wk.init(s, n_items, blocks_per_seq, true); wk.ok; wk.next(s, n_items, blocks_per_seq, true)) {
+        for (wk.init(s, n_items, blocks_per_seq, kTileRows, true); wk.ok; wk.next(s)) {
           if (wk.j == 0) {
             const int qb = wk.k & 1;
             mbar_wait(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
@@ -108,7 +108,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     } else if (warp == 9) {
       // ------------------------------------------------------------------ MMA issuer
       Walker a, p;  // a: S issue (one tile ahead), p: PV issue
-      a.init(s, n_items, blocks_per_seq, true);
+      a.init(s, n_items, blocks_per_seq, kTileRows, true);
       p = a;
       auto issue_s = [&]() {
         const int qb = a.k & 1, st = a.t % ST;
@@ -127,7 +127,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           if (a.j == a.tiles - 1) tc_commit(smem_u32(&bar_q_empty[qb]));
         }
         __syncwarp();
-        a.next(s, n_items, blocks_per_seq, true);
+        a.next(s);
       };
       auto issue_o = [&]() {
         const int st = p.t % ST;
@@ -145,7 +145,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           tc_commit(smem_u32(&bar_kv_empty[st]));
         }
         __syncwarp();
-        p.next(s, n_items, blocks_per_seq, true);
+        p.next(s);
       };
       if (a.ok) issue_s();
       while (p.ok) {
@@ -168,9 +168,10 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     uint32_t g = 0;  // tiles processed by this CTA so far
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       Walker it;
+      it.n_items = n_items; it.bps = blocks_per_seq; it.chunk = kTileRows; it.over_keys = true;
       it.w = w;
       bool valid;
-      it.decode(s, blocks_per_seq, valid);
+      it.decode(s, valid);
       const int row = it.blk * 2 * kTileRows + t * kTileRows + r;
       __nv_bfloat16* orow = O + (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
       float* lse = LSE + (((size_t)it.b * s.C + it.c) * s.H + it.h) * s.R + row;
