@@ -1,8 +1,9 @@
 // Item-axis dispatch: picks the tcgen05 kernels (item_tc_*.cu) or the SIMT bring-up kernels
 // (item_simt.cu) for a shape and owns the workspace layout.  SURVEY.md §8(a) rows a3-a5.
 //
-// Workspace of tabattn_item_bwd: D = rowsum(dO o O) as f32 [B,C,H,R] (written by the dQ pass,
-// read by the dK/dV pass).  tabattn_item_fwd needs none.
+// Workspace of tabattn_item_bwd: two f32 arrays [B*C*H][Rp] (Rp = R rounded up to 64), written by
+// the prep kernel and read by both passes: lse2 = LSE * log2(e) and D = rowsum(dO o O).
+// tabattn_item_fwd needs none.
 #include <stdlib.h>
 #include <string.h>
 
@@ -19,6 +20,7 @@ cudaError_t launch_item_bwd_simt(const Shape& s, const void* Q, const void* K, c
 // item_tc_fwd.cu / item_tc_bwd.cu
 bool item_tc_supported(const Shape& s);
 bool item_tc_bwd_supported(const Shape& s);
+int item_bwd_padded_rows(const Shape& s);
 cudaError_t launch_item_fwd_tc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                cudaStream_t stream);
 cudaError_t launch_item_bwd_tc(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
@@ -36,7 +38,7 @@ bool force_simt() {
 size_t item_fwd_workspace_bytes(const Shape&) { return 0; }
 
 size_t item_bwd_workspace_bytes(const Shape& s) {
-  return (size_t)s.B * s.C * s.H * s.R * sizeof(float);
+  return (size_t)2 * s.B * s.C * s.H * item_bwd_padded_rows(s) * sizeof(float);
 }
 
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,

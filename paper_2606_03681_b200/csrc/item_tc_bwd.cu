@@ -1,6 +1,9 @@
-// Item-axis attention backward on tcgen05: the dQ pass (which
-// also emits D = rowsum(dO o O)) and the separate dK/dV pass, one kernel template with two modes.
-// Deterministic: no atomics, every output element has exactly one writer.
+// Item-axis attention backward on tcgen05: a small prep kernel
+// (D = rowsum(dO o O) and LSE in log2 units, into the workspace), the dQ pass and the separate
+// dK/dV pass -- one kernel template with two modes.  Deterministic: no atomics, every output
+// element has exactly one writer.  (The split costs one extra exp and two extra tile-matmuls per
+// (query, key) pair over a fused pass, but a fused pass must reduce dQ across key tiles with fp32
+// atomics: at dh = 32/64 that is 8-16 B of L2 atomic traffic per 10*dh flops -- see DESIGN.md.)
 //
 // Both passes have the same shape: a STATIONARY 128-row tile pair (A1, A2) against a STREAM of
 // 64-row chunk pairs (B1, B2):
@@ -11,10 +14,16 @@
 // with P = exp2(S * scale*log2e - LSE*log2e) recomputed from the saved LSE.  S/dP accumulate in
 // TMEM (fp32); P and dS go back to TMEM as bf16 and are the A operands of the second-stage MMAs.
 //
-// Warp roles (384 threads, one persistent CTA per SM): warp 8 TMA producer (+ LSE/D chunk staging in
-// MODE_DKV), warp 9 MMA issuer, warpgroups 0/1 = "set" 0/1: each owns one TMEM set (S, dP, dS, P) and
-// takes every other chunk, one thread per tile row; the score MMAs run up to three chunks ahead of the
-// accumulation MMAs, across item boundaries.
+// Warp roles (384 threads, one persistent CTA per SM):
+//   warp 8   TMA producer (one lane): stationary tiles (double-buffered over items), ring of chunk
+//            pairs (+ the chunk's LSE/D vectors by 1-D bulk copy in MODE_DKV)
+//   warp 9   issuer of the score MMAs (S, dP), two chunks ahead of the accumulation MMAs
+//   warp 10  issuer of the accumulation MMAs (one lane); owns the TMEM allocation
+//   warpgroups 0/1 = "set" 0/1: each owns one TMEM set (S, dP, dS, P) and takes every other chunk,
+//            one thread per tile row.
+// Every role walks the same item list with its own counters; the per-chunk work of the single-lane
+// roles is a few waits plus the MMA/TMA issues on precomputed descriptors (the first build of this
+// file was bound by the issue rate of its one MMA warp, profiles/r01_tc_launches.md).
 #include <cuda.h>
 
 #include <algorithm>
@@ -23,6 +32,8 @@
 #include "kernels.h"
 
 namespace tabattn {
+
+int item_bwd_padded_rows(const Shape& s);
 
 namespace {
 
@@ -38,31 +49,102 @@ struct BwdCfg {
   static constexpr int ROWB = DH * 2;
   static constexpr int TILE_A = kTileRows * ROWB;  // stationary tile
   static constexpr int TILE_B = kChunk * ROWB;     // streamed chunk
-  static constexpr int ST = 4;                     // chunk ring depth
+  static constexpr int ST = 6;                     // chunk ring depth
   static constexpr int LD_BYTES = 2 * kChunk * 4;  // per stage: lse2[64], D[64] (MODE_DKV)
-  static constexpr int SMEM = 4 * TILE_A + ST * (2 * TILE_B + LD_BYTES) + 1024;
+  static constexpr int STAGE = 2 * TILE_B;         // bytes of one ring stage (B1, B2)
+  static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + 1024;
   // TMEM columns: set g at g*SET: S [0,64) dP [64,128) dS [128,160) P [160,192); accumulators after
   static constexpr int SET = 192, S_OFF = 0, DP_OFF = 64, DS_OFF = 128, P_OFF = 160;
   static constexpr int ACC0 = 384, ACC1 = 384 + DH, COLS = 512;
   static_assert(ACC1 + DH <= COLS, "TMEM budget");
 };
 
+// One work item = (table b, column c, head h, 128-row block blk) of the stationary axis.
+struct Item {
+  int b, c, h, blk, n, chunks;
+  bool valid;
+};
+
+template <int MODE>
+__device__ __forceinline__ Item decode_item(const Shape& s, int w, int bps) {
+  Item it;
+  it.blk = w % bps;
+  const int rest = w / bps;
+  it.h = rest % s.H;
+  const int bc = rest / s.H;
+  it.b = bc / s.C;
+  it.c = bc - it.b * s.C;
+  it.n = clamp_n(s, it.b);
+  it.valid = (!s.col_valid || __ldg(s.col_valid + bc) != 0) && (MODE == MODE_DQ || it.blk * kTileRows < it.n);
+  it.chunks = ((MODE == MODE_DQ ? it.n : s.R) + kChunk - 1) / kChunk;
+  return it;
+}
+
+// 1-D bulk copy global -> shared, completion on an mbarrier (bytes multiple of 16, both 16 B aligned)
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+
+// ---- prep: D[b,c,h,r] = sum_k dO O, lse2 = LSE * log2(e); rows r in [R, Rp) get D = 0, lse2 = +inf ------
+// One CTA = 32 rows of one (b, c); the two outputs are [B*C*H][Rp] f32 (Rp = R rounded up to 64).
+__global__ void __launch_bounds__(256) item_bwd_prep_kernel(Shape s, const __nv_bfloat16* __restrict__ O,
+                                                            const __nv_bfloat16* __restrict__ dO,
+                                                            const float* __restrict__ LSE,
+                                                            float* __restrict__ lse2_ws, float* __restrict__ D_ws,
+                                                            int Rp) {
+  __shared__ float sD[32][33];
+  const int bc = blockIdx.y, b = bc / s.C, c = bc - b * s.C;
+  if (s.col_valid && __ldg(s.col_valid + bc) == 0) return;
+  const int r0 = blockIdx.x * 32;
+  const int d = s.H * s.dh, vpr = d / 8, vph = s.dh / 8;
+  for (int i = threadIdx.x; i < 32 * 33; i += 256) (&sD[0][0])[i] = 0.f;
+  __syncthreads();
+  // 32 * vpr is a multiple of 32, so whole warps enter or leave the loop together (the shuffles below
+  // need every lane); rows >= R contribute 0 instead of branching around them.
+  for (int idx = threadIdx.x; idx < 32 * vpr; idx += 256) {
+    const int rr = idx / vpr, v = idx - rr * vpr, r = r0 + rr;
+    float a = 0.f;
+    if (r < s.R) {
+      const size_t off = (((size_t)b * s.R + r) * s.C + c) * d + 8 * v;
+      float fo[8], fg[8];
+      unpack8(ldg_nc_v4(O + off), fo);
+      unpack8(ldg_nc_v4(dO + off), fg);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) a = fmaf(fo[e], fg[e], a);
+    }
+    // the vph partial sums of one (row, head) sit in vph consecutive lanes (vpr is a multiple of
+    // vph = 2, 4 or 8): butterfly-add them, a fixed order
+    for (int o = 1; o < vph; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if ((v % vph) == 0) sD[rr][v / vph] = a;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < 32 * s.H; idx += 256) {
+    const int h = idx >> 5, rr = idx & 31, r = r0 + rr;
+    if (r >= Rp) continue;
+    const size_t seq = ((size_t)bc * s.H + h);
+    const bool in = r < s.R;
+    lse2_ws[seq * Rp + r] = in ? __ldg(LSE + seq * s.R + r) * kLog2e : INFINITY;
+    D_ws[seq * Rp + r] = in ? sD[rr][h] : 0.f;
+  }
+}
+
 template <int DH, int MODE>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_constant__ CUtensorMap mapA2,
                    const __grid_constant__ CUtensorMap mapB1, const __grid_constant__ CUtensorMap mapB2, Shape s,
-                   const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __restrict__ dO,
-                   const float* __restrict__ LSE, float* __restrict__ Dws, __nv_bfloat16* __restrict__ out0,
-                   __nv_bfloat16* __restrict__ out1, int n_items, int blocks_per_seq) {
+                   const float* __restrict__ lse2_ws, const float* __restrict__ D_ws,
+                   __nv_bfloat16* __restrict__ out0, __nv_bfloat16* __restrict__ out1, int n_items,
+                   int blocks_per_seq, int Rp) {
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE_A = Cfg::TILE_A, TILE_B = Cfg::TILE_B, ROWB = Cfg::ROWB;
-  constexpr bool kOverKeys = MODE == MODE_DQ;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = sbase;                         // [2 item buffers][A1, A2][TILE_A]
   const uint32_t sB = sA + 4 * TILE_A;               // [ST][B1, B2][TILE_B]
-  const uint32_t sLD = sB + ST * 2 * TILE_B;         // [ST][lse2[64], D[64]]
-  float* sLD_ptr = reinterpret_cast<float*>(smem_raw + (sLD - smem_u32(smem_raw)));
+  const uint32_t sLD = sB + ST * Cfg::STAGE;         // [ST][lse2[64], D[64]]
+  const float* sLD_ptr = reinterpret_cast<const float*>(smem_raw + (sLD - smem_u32(smem_raw)));
   __shared__ uint64_t bar_a_full[2], bar_a_empty[2], bar_b_full[ST], bar_b_empty[ST];
   __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_p_empty[2], bar_acc_full, bar_acc_free;
   __shared__ uint32_t tmem_slot;
@@ -74,16 +156,16 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       mbar_init(smem_u32(&bar_a_full[i]), 1);
       mbar_init(smem_u32(&bar_a_empty[i]), 1);
       mbar_init(smem_u32(&bar_s_full[i]), 1);
-      mbar_init(smem_u32(&bar_s_empty[i]), 128);
-      mbar_init(smem_u32(&bar_p_full[i]), 128);
+      mbar_init(smem_u32(&bar_s_empty[i]), 4);   // one arrive per warp of the set's warpgroup
+      mbar_init(smem_u32(&bar_p_full[i]), 4);
       mbar_init(smem_u32(&bar_p_empty[i]), 1);
     }
     for (int i = 0; i < ST; ++i) {
-      mbar_init(smem_u32(&bar_b_full[i]), MODE == MODE_DKV ? 2 : 1);
+      mbar_init(smem_u32(&bar_b_full[i]), 1);
       mbar_init(smem_u32(&bar_b_empty[i]), 1);
     }
     mbar_init(smem_u32(&bar_acc_full), 1);
-    mbar_init(smem_u32(&bar_acc_free), 256);
+    mbar_init(smem_u32(&bar_acc_free), 8);
     fence_barrier_init();
   }
   tc_fence_before();
@@ -92,109 +174,113 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   const uint32_t tmem = tmem_slot;
   const int d = s.H * DH;
 
-  if (warp >= 8) {
-    setmaxnreg_dec<56>();
-    if (warp == 8) {
-      // ------------------------------------------------------------------ producer
-      if (lane == 0) {
-        tma_prefetch_desc(&mapA1);
-        tma_prefetch_desc(&mapA2);
-        tma_prefetch_desc(&mapB1);
-        tma_prefetch_desc(&mapB2);
-      }
-      Walker wk;
-      for (wk.init(s, n_items, blocks_per_seq, kChunk, kOverKeys); wk.ok; wk.next(s)) {
-        const int st = wk.t % ST;
-        if (lane == 0) {
-          if (wk.j == 0) {
-            const int ab = wk.k & 1;
-            mbar_wait(smem_u32(&bar_a_empty[ab]), ((wk.k >> 1) & 1) ^ 1);
-            mbar_arrive_expect_tx(smem_u32(&bar_a_full[ab]), 2 * TILE_A);
-            tma_load_5d(sA + (2 * ab) * TILE_A, &mapA1, smem_u32(&bar_a_full[ab]), 0, wk.h, wk.c,
-                        wk.blk * kTileRows, wk.b);
-            tma_load_5d(sA + (2 * ab + 1) * TILE_A, &mapA2, smem_u32(&bar_a_full[ab]), 0, wk.h, wk.c,
-                        wk.blk * kTileRows, wk.b);
+  if (warp == 8) {
+    // ------------------------------------------------------------------ producer (one lane)
+    if (lane == 0) {
+      tma_prefetch_desc(&mapA1);
+      tma_prefetch_desc(&mapA2);
+      tma_prefetch_desc(&mapB1);
+      tma_prefetch_desc(&mapB2);
+      uint32_t t = 0, k = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+        const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+        if (!it.valid) continue;
+        const uint32_t ab = k & 1, a_full = smem_u32(&bar_a_full[ab]);
+        mbar_wait(smem_u32(&bar_a_empty[ab]), ((k >> 1) & 1) ^ 1);
+        mbar_arrive_expect_tx(a_full, 2 * TILE_A);
+        tma_load_5d(sA + (2 * ab) * TILE_A, &mapA1, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
+        tma_load_5d(sA + (2 * ab + 1) * TILE_A, &mapA2, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
+        const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
+        for (int j = 0; j < it.chunks; ++j, ++t) {
+          const uint32_t st = t % ST, b_full = smem_u32(&bar_b_full[st]);
+          mbar_wait(smem_u32(&bar_b_empty[st]), ((t / ST) & 1) ^ 1);
+          mbar_arrive_expect_tx(b_full, Cfg::STAGE + (MODE == MODE_DKV ? Cfg::LD_BYTES : 0));
+          tma_load_5d(sB + st * Cfg::STAGE, &mapB1, b_full, 0, it.h, it.c, j * kChunk, it.b);
+          tma_load_5d(sB + st * Cfg::STAGE + TILE_B, &mapB2, b_full, 0, it.h, it.c, j * kChunk, it.b);
+          if (MODE == MODE_DKV) {
+            bulk_load(sLD + st * Cfg::LD_BYTES, lse2_ws + seq + j * kChunk, kChunk * 4, b_full);
+            bulk_load(sLD + st * Cfg::LD_BYTES + kChunk * 4, D_ws + seq + j * kChunk, kChunk * 4, b_full);
           }
-          mbar_wait(smem_u32(&bar_b_empty[st]), ((wk.t / ST) & 1) ^ 1);
-          mbar_arrive_expect_tx(smem_u32(&bar_b_full[st]), 2 * TILE_B);
-          tma_load_5d(sB + (2 * st) * TILE_B, &mapB1, smem_u32(&bar_b_full[st]), 0, wk.h, wk.c, wk.j * kChunk, wk.b);
-          tma_load_5d(sB + (2 * st + 1) * TILE_B, &mapB2, smem_u32(&bar_b_full[st]), 0, wk.h, wk.c, wk.j * kChunk,
-                      wk.b);
         }
-        if (MODE == MODE_DKV) {
-          __syncwarp();  // lane 0 has seen the stage free
-          const size_t seq = (((size_t)wk.b * s.C + wk.c) * s.H + wk.h) * s.R;
-          float* ld = sLD_ptr + st * (2 * kChunk);
-#pragma unroll
-          for (int e = 0; e < kChunk / 32; ++e) {
-            const int i = wk.j * kChunk + 32 * e + lane;
-            const bool in = i < s.R;
-            ld[32 * e + lane] = in ? __ldg(LSE + seq + i) * kLog2e : INFINITY;
-            ld[kChunk + 32 * e + lane] = in ? __ldg(Dws + seq + i) : 0.f;
-          }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&bar_b_full[st]));
-        }
+        ++k;
       }
-    } else if (warp == 9) {
-      // ------------------------------------------------------------------ MMA issuer
-      // a: score MMAs (up to three chunks ahead), p: accumulation MMAs.  Chunk t of the CTA's
-      // lifetime uses TMEM set t & 1 (global alternation: consecutive chunks never share a set, also
-      // across items, so a score issue never waits on a warpgroup that is itself waiting for an
-      // accumulation MMA that is issued later); it is that set's (t >> 1)-th chunk.
-      Walker a, p;
-      a.init(s, n_items, blocks_per_seq, kChunk, kOverKeys);
-      p = a;
-      auto issue_scores = [&]() {
-        const int ab = a.k & 1, st = a.t % ST, g = a.t & 1;
-        if (a.j == 0) mbar_wait(smem_u32(&bar_a_full[ab]), (a.k >> 1) & 1);
-        mbar_wait(smem_u32(&bar_b_full[st]), (a.t / ST) & 1);
+    }
+  } else if (warp == 9) {
+    // ------------------------------------------------------------------ score MMAs (S, dP)
+    // Chunk t of the CTA's lifetime uses TMEM set t & 1 and ring stage t % ST.  The whole warp walks
+    // the loop (the tail zeroing needs all lanes); lane 0 issues.
+    constexpr uint32_t idesc = make_idesc_bf16(128, kChunk, false, false);
+    const uint64_t dA = make_smem_desc<ROWB>(sA, 16, 8 * ROWB);
+    const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
+    uint32_t t = 0, k = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+      if (!it.valid) continue;
+      const uint32_t ab = k & 1;
+      mbar_wait(smem_u32(&bar_a_full[ab]), (k >> 1) & 1);
+      const uint64_t a1 = dA + ((2 * ab) * TILE_A >> 4), a2 = a1 + (TILE_A >> 4);
+      for (int j = 0; j < it.chunks; ++j, ++t) {
+        const uint32_t st = t % ST, g = t & 1;
+        mbar_wait(smem_u32(&bar_b_full[st]), (t / ST) & 1);
         if (MODE == MODE_DQ) {
-          const int rem = a.n - a.j * kChunk;  // keys >= n must not reach dQ through dS K
-          if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + (2 * st) * TILE_B, rem, lane);
+          const int rem = it.n - j * kChunk;  // keys >= n must not reach dQ through dS K
+          if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
         if (lane == 0) {
-          mbar_wait(smem_u32(&bar_s_empty[g]), ((a.t >> 1) & 1) ^ 1);
+          mbar_wait(smem_u32(&bar_s_empty[g]), ((t >> 1) & 1) ^ 1);
           tc_fence_after();
           const uint32_t set = tmem + g * Cfg::SET;
-          issue_qk<DH, kChunk>(set + Cfg::S_OFF, sA + (2 * ab) * TILE_A, sB + (2 * st) * TILE_B);
-          issue_qk<DH, kChunk>(set + Cfg::DP_OFF, sA + (2 * ab + 1) * TILE_A, sB + (2 * st + 1) * TILE_B);
+          const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
+#pragma unroll
+          for (int kk = 0; kk < DH / 16; ++kk) mma_ss(set + Cfg::S_OFF, a1 + 2 * kk, b1 + 2 * kk, idesc, kk > 0);
+#pragma unroll
+          for (int kk = 0; kk < DH / 16; ++kk) mma_ss(set + Cfg::DP_OFF, a2 + 2 * kk, b2 + 2 * kk, idesc, kk > 0);
           tc_commit(smem_u32(&bar_s_full[g]));
-          if (a.j == a.tiles - 1) tc_commit(smem_u32(&bar_a_empty[ab]));
+          if (j == it.chunks - 1) tc_commit(smem_u32(&bar_a_empty[ab]));
         }
         __syncwarp();
-        a.next(s);
-      };
-      auto issue_acc = [&]() {
-        const int st = p.t % ST, g = p.t & 1;
-        if (lane == 0) {
-          if (p.j == 0) mbar_wait(smem_u32(&bar_acc_free), (p.k & 1) ^ 1);
-          mbar_wait(smem_u32(&bar_p_full[g]), (p.t >> 1) & 1);
+      }
+      ++k;
+    }
+  } else if (warp == 10) {
+    // ------------------------------------------------------------------ accumulation MMAs (one lane)
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(128, DH, false, true);
+      const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
+      uint32_t t = 0, k = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+        const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+        if (!it.valid) continue;
+        mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
+        for (int j = 0; j < it.chunks; ++j, ++t) {
+          const uint32_t st = t % ST, g = t & 1;
+          mbar_wait(smem_u32(&bar_p_full[g]), (t >> 1) & 1);
           tc_fence_after();
           const uint32_t set = tmem + g * Cfg::SET;
+          const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
+          // A = 128 x 64 bf16 in TMEM (8 columns per 16-wide k step); B = 16 chunk rows per k step
           if (MODE == MODE_DQ) {
-            issue_pv<DH, kChunk>(tmem + Cfg::ACC0, set + Cfg::DS_OFF, sB + (2 * st) * TILE_B, p.j > 0);
+#pragma unroll
+            for (int kk = 0; kk < kChunk / 16; ++kk)
+              mma_ts(tmem + Cfg::ACC0, set + Cfg::DS_OFF + 8 * kk, b1 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
           } else {
-            issue_pv<DH, kChunk>(tmem + Cfg::ACC0, set + Cfg::P_OFF, sB + (2 * st + 1) * TILE_B, p.j > 0);
-            issue_pv<DH, kChunk>(tmem + Cfg::ACC1, set + Cfg::DS_OFF, sB + (2 * st) * TILE_B, p.j > 0);
+#pragma unroll
+            for (int kk = 0; kk < kChunk / 16; ++kk)
+              mma_ts(tmem + Cfg::ACC0, set + Cfg::P_OFF + 8 * kk, b2 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
+#pragma unroll
+            for (int kk = 0; kk < kChunk / 16; ++kk)
+              mma_ts(tmem + Cfg::ACC1, set + Cfg::DS_OFF + 8 * kk, b1 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
           }
           tc_commit(smem_u32(&bar_p_empty[g]));
           tc_commit(smem_u32(&bar_b_empty[st]));
-          if (p.j == p.tiles - 1) tc_commit(smem_u32(&bar_acc_full));
+          if (j == it.chunks - 1) tc_commit(smem_u32(&bar_acc_full));
         }
-        __syncwarp();
-        p.next(s);
-      };
-      if (a.ok) issue_scores();
-      if (a.ok) issue_scores();
-      while (p.ok) {
-        if (a.ok) issue_scores();
-        issue_acc();
+        ++k;
       }
     }
-  } else {
+    __syncwarp();
+  } else if (warp < 8) {
     // -------------------------------------------------------------------- score warpgroups (sets)
-    setmaxnreg_inc<224>();
     const int g = warp >> 2;                 // TMEM set / chunk parity of this warpgroup
     const int r = threadIdx.x & 127;         // tile row = TMEM lane
     const uint32_t lane_base = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
@@ -204,22 +290,17 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     const float c2 = s.scale * kLog2e;
     uint32_t kitem = 0;   // valid items seen
     uint32_t tbase = 0;   // chunks of all previous valid items (ring position)
-    Walker it;
-    it.n_items = n_items; it.bps = blocks_per_seq; it.chunk = kChunk; it.over_keys = kOverKeys;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      it.w = w;
-      bool valid;
-      it.decode(s, valid);
+      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       const int row = it.blk * kTileRows + r;
       const size_t cell = (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
-      const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * s.R;
-      if (!valid) {
+      const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
+      if (!it.valid) {
         // invalid column, or (MODE_DKV) a key block entirely beyond the train rows: zeros
         if (row < s.R) {
           if (MODE == MODE_DQ) {
 #pragma unroll
             for (int k = 0; k < DH / 16; ++k) stg_v4(out0 + cell + g * (DH / 2) + 8 * k, make_uint4(0, 0, 0, 0));
-            if (g == 0) Dws[seq + row] = 0.f;
           } else {
             __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell;
 #pragma unroll
@@ -228,21 +309,13 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         }
         continue;
       }
-      // per-row constants of the dQ pass: LSE_i and D_i = sum_k dO_ik O_ik (also saved for the dK/dV pass)
+      // per-row constants of the dQ pass (rows >= R: lse2 = +inf -> P = 0)
       float lse2 = INFINITY, Drow = 0.f;
-      if (MODE == MODE_DQ && row < s.R) {
-        lse2 = __ldg(LSE + seq + row) * kLog2e;
-#pragma unroll
-        for (int k = 0; k < DH / 8; ++k) {
-          float fo[8], fg[8];
-          unpack8(ldg_nc_v4(O + cell + 8 * k), fo);
-          unpack8(ldg_nc_v4(dO + cell + 8 * k), fg);
-#pragma unroll
-          for (int e = 0; e < 8; ++e) Drow = fmaf(fo[e], fg[e], Drow);
-        }
-        if (g == 0) Dws[seq + row] = Drow;
+      if (MODE == MODE_DQ && row < Rp) {
+        lse2 = __ldg(lse2_ws + seq + row);
+        Drow = __ldg(D_ws + seq + row);
       }
-      const int chunks = it.tiles;
+      const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
         mbar_wait(b_s_full, u & 1);
@@ -254,7 +327,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         tmem_ld32(set + Cfg::DP_OFF + 32, dr + 32);
         tmem_wait_ld();
         tc_fence_before();
-        mbar_arrive(b_s_empty);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_s_empty);
         uint32_t pds[32], pp[32];
         if (MODE == MODE_DQ) {
           const int rem = it.n - j * kChunk;
@@ -272,7 +346,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           }
         } else {
           const uint32_t st = (tbase + j) % ST;
-          mbar_wait(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);  // LSE/D chunk is visible
+          // the chunk's LSE/D vectors landed with the chunk (same mbarrier as the score MMAs waited on)
+          mbar_wait(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
           const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + st * (2 * kChunk));
           const float4* d4 = l4 + kChunk / 4;
 #pragma unroll
@@ -294,7 +369,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         if (MODE == MODE_DKV) tmem_st32(set + Cfg::P_OFF, pp);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(b_p_full);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_p_full);
       }
       // ---- epilogue ---------------------------------------------------------------------------------
       mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
@@ -304,7 +380,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         uint32_t acc[HALF];
         tmem_ld_cols<HALF>(lane_base + Cfg::ACC0 + g * HALF, acc);
         tc_fence_before();
-        mbar_arrive(smem_u32(&bar_acc_free));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
         if (row < s.R) {
 #pragma unroll
           for (int k = 0; k < HALF / 8; ++k) {
@@ -318,9 +395,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         uint32_t acc[DH];  // warpgroup 0: dV = acc0; warpgroup 1: dK = scale * acc1
         tmem_ld_cols<DH>(lane_base + (g == 0 ? Cfg::ACC0 : Cfg::ACC1), acc);
         tc_fence_before();
-        mbar_arrive(smem_u32(&bar_acc_free));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
         if (row < s.R) {
-          const float mul = row < it.n ? (g == 0 ? 1.f : s.scale) : 0.f;
+          const float mul = g == 0 ? 1.f : s.scale;
           __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell;
 #pragma unroll
           for (int k = 0; k < DH / 8; ++k) {
@@ -342,7 +420,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
 
 template <int DH>
 cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O, const void* dO,
-                       const float* LSE, void* dQ, void* dK, void* dV, float* Dws, cudaStream_t stream) {
+                       const float* LSE, void* dQ, void* dK, void* dV, float* ws, cudaStream_t stream) {
   using Cfg = BwdCfg<DH>;
   CUtensorMap q128, g128, k128, v128, q64, g64, k64, v64;
   bool ok = make_cell_tensor_map(&q128, Q, s.B, s.R, s.C, s.H, DH, kTileRows) &&
@@ -363,16 +441,19 @@ cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void*
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
+  const int Rp = item_bwd_padded_rows(s);
+  float* lse2_ws = ws;
+  float* D_ws = ws + (size_t)s.B * s.C * s.H * Rp;
+  item_bwd_prep_kernel<<<dim3(Rp / 32, s.B * s.C), 256, 0, stream>>>(s, (const __nv_bfloat16*)O,
+                                                                     (const __nv_bfloat16*)dO, LSE, lse2_ws, D_ws, Rp);
   const int bps = (s.R + kTileRows - 1) / kTileRows;
   const long long n_items = (long long)s.B * s.C * s.H * bps;
   const int grid = (int)std::min<long long>(n_items, num_sms());
-  const __nv_bfloat16* Ob = (const __nv_bfloat16*)O;
-  const __nv_bfloat16* dOb = (const __nv_bfloat16*)dO;
-  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, s, Ob, dOb, LSE, Dws, (__nv_bfloat16*)dQ,
-                                               nullptr, (int)n_items, bps);
-  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, s, Ob, dOb, LSE, Dws, (__nv_bfloat16*)dV,
-                                                (__nv_bfloat16*)dK, (int)n_items, bps);
-  count_launch(2);
+  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, s, lse2_ws, D_ws, (__nv_bfloat16*)dQ, nullptr,
+                                               (int)n_items, bps, Rp);
+  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, s, lse2_ws, D_ws, (__nv_bfloat16*)dV,
+                                                (__nv_bfloat16*)dK, (int)n_items, bps, Rp);
+  count_launch(3);
   return cudaGetLastError();
 }
 
@@ -380,13 +461,17 @@ cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void*
 
 bool item_tc_bwd_supported(const Shape& s) { return s.dh == 16 || s.dh == 32 || s.dh == 64; }
 
+// rows of the per-sequence LSE/D workspace vectors: R rounded up to the 64-row chunk, so that every
+// chunk's vectors are one aligned 256-byte bulk copy
+int item_bwd_padded_rows(const Shape& s) { return (s.R + kChunk - 1) / kChunk * kChunk; }
+
 cudaError_t launch_item_bwd_tc(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
-                               const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* Dws,
+                               const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
                                cudaStream_t stream) {
   switch (s.dh) {
-    case 16: return launch_bwd<16>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, Dws, stream);
-    case 32: return launch_bwd<32>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, Dws, stream);
-    case 64: return launch_bwd<64>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, Dws, stream);
+    case 16: return launch_bwd<16>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, stream);
+    case 32: return launch_bwd<32>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, stream);
+    case 64: return launch_bwd<64>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, stream);
     default: return cudaErrorInvalidValue;
   }
 }
