@@ -2,9 +2,11 @@
 //
 // The feature axis is short (C <= 128 columns) and the path is HBM-bound (0.58*C flop/B), so the
 // kernels are built around the memory stream, not around the contraction:
-//   * persistent CTAs of 4 warps, several per SM; every CTA walks "stage units" = (table b, block of
+//   * persistent CTAs of 3-8 warps, several per SM; every CTA walks "stage units" = (table b, block of
 //     `rows` table rows, group of `hg` heads) and keeps a ring of NSTAGE stages in flight with
-//     16-byte cp.async (LDGSTS) copies -- one stage is being computed while the next ones land;
+//     16-byte cp.async (LDGSTS) copies -- one stage is being computed while the next ones land.
+//     (One 1-D bulk copy per cell was measured first: the TMA unit retires one cp.async.bulk per
+//     ~68 clk per SM whatever its size, 3x too slow for 384-byte cells: profiles/r01_feature_mma.md);
 //   * only VALID columns are loaded (gathered): the cells of a row are compacted to slots
 //     v = 0..Cv-1 in shared memory, so DRAM traffic equals the algorithmic bytes even under a mask;
 //     each cell slot is padded by 16 B, which makes every ldmatrix phase hit 8 distinct 16-byte
@@ -25,21 +27,21 @@
 #include "common.cuh"
 #include "kernels.h"
 
+#include <stdio.h>
 #include <stdlib.h>
 
 namespace tabattn {
 
 namespace {
 
-constexpr int kWarps = 4;
-constexpr int kThreads = kWarps * 32;
+constexpr int kMaxWarps = 8;
 constexpr int kMaxStages = 4;
 
 struct FeatParams {
   Shape s;
   int hg, nhg;          // heads per stage unit, units per (table, row block)
   int rows;             // table rows per stage unit
-  int Cp;               // cell slots per table row: C rounded up to 16
+  int Cp;               // C rounded up to 16: pitch of the per-(row, head) statistics vectors
   int slot_stride;      // bytes per cell slot: hg*dh*2 + 16
   int chunks;           // 16-byte chunks per cell slot payload: hg*dh/8
   int rb_per_table;     // ceil(R / rows)
@@ -51,6 +53,7 @@ struct FeatParams {
   uint32_t off_lse, off_D, off_vcol, off_cv, stage_bytes;  // layout of one stage
   uint32_t stage0;      // offset of stage 0 (after the per-warp staging tiles)
   int nstage;
+  int ld_dcell, ld_dch; // loader step of one CTA-wide stride: nthreads / chunks, nthreads % chunks
 };
 
 // x / d for x < 2^32 / d with magic = floor(2^32 / d) + 1 (0 stands for d == 1)
@@ -133,7 +136,10 @@ struct ColMask {
   uint32_t m[4];
   int below[4];
   int Cv;
-  __device__ __forceinline__ void build(const Shape& s, int b) {
+  int b = -1;   // table the mask was built for (the walker revisits a table for many stages)
+  __device__ __forceinline__ void build(const Shape& s, int b_) {
+    if (b_ == b) return;
+    b = b_;
     const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -159,45 +165,78 @@ struct ColMask {
   }
 };
 
+
+// Per-lane byte offsets of the three ldmatrix address patterns (slot stride `str`), computed once.
+struct LaneOff {
+  uint32_t a;    // A fragment, 16 rows x 16 k:      row = lane & 15,                 col = (lane >> 4) * 16 B
+  uint32_t nb;   // B fragment from an [n][k] tile:  row = (lane & 7) + 8*(lane >> 4), col = ((lane >> 3) & 1) * 16 B
+  uint32_t tb;   // B fragment from a [k][n] tile (.trans): row = (lane & 7) + 8*((lane >> 3) & 1), col = (lane >> 4) * 16 B
+  __device__ __forceinline__ void init(int str) {
+    const int lane = threadIdx.x & 31;
+    a = (lane & 15) * str + (lane >> 4) * 16;
+    nb = ((lane & 7) + ((lane >> 4) << 3)) * str + ((lane >> 3) & 1) * 16;
+    tb = ((lane & 7) + (((lane >> 3) & 1) << 3)) * str + (lane >> 4) * 16;
+  }
+};
+
 // ---- stage loader ------------------------------------------------------------------------------------
-// Issues the cp.async copies of one stage unit into ring buffer `stage` (shared-memory byte address)
-// and zero-fills the outputs of the unit's invalid cells.  NIN input tensors share one offset map.
-// Called by all threads of the CTA (uniformly); the caller commits the group.
+// Issues the 16-byte cp.async copies of one stage unit into ring buffer `stage` (shared byte address):
+// valid cell (r, c) -> compacted, padded slot (r*Cv + rank(c)); zero-fills the outputs of invalid cells
+// (a6); (backward) fetches the saved LSE of the valid triples.  All threads of the CTA call it,
+// uniformly; the caller commits the group.
 template <int NIN, int NOUT, bool BWD>
-__device__ __forceinline__ void issue_stage(const FeatParams& p, const Unit& u, uint32_t stage, unsigned char* stage_ptr,
-                                            const unsigned char* const (&in)[NIN], unsigned char* const (&out)[NOUT],
-                                            float* __restrict__ LSE_out, const float* __restrict__ LSE_in) {
+__device__ __forceinline__ void issue_stage(const FeatParams& p, const Unit& u, ColMask& cm, uint32_t stage,
+                                            unsigned char* stage_ptr, const unsigned char* const (&in)[NIN],
+                                            unsigned char* const (&out)[NOUT], float* __restrict__ LSE_out,
+                                            const float* __restrict__ LSE_in) {
   const Shape& s = p.s;
-  ColMask cm;
   cm.build(s, u.b);
-  const int d2 = s.H * s.dh * 2;                    // bytes per cell
-  const int hoff = u.hgi * p.hg * s.dh * 2;         // byte offset of the head group inside a cell
+  const uint32_t d2 = s.H * s.dh * 2;                    // bytes per cell
+  const uint32_t hoff = u.hgi * p.hg * s.dh * 2;         // byte offset of the head group inside a cell
   const size_t row0 = (size_t)u.b * s.R + u.r0;
-  const uint32_t total = (uint32_t)u.nrows * s.C * p.chunks;
-  for (uint32_t idx = threadIdx.x; idx < total; idx += kThreads) {
-    const uint32_t cellidx = fdiv(idx, p.div_chunks);
-    const uint32_t ch = idx - cellidx * p.chunks;
-    const uint32_t r = fdiv(cellidx, p.div_C);
-    const int c = (int)(cellidx - r * s.C);
-    const size_t goff = ((row0 + r) * s.C + c) * (size_t)d2 + hoff + ch * 16;
-    if (cm.valid(c)) {
-      const int v = cm.rank(c);
-      const uint32_t soff = (r * p.Cp + v) * p.slot_stride + ch * 16;
+  const size_t gbase = row0 * s.C * (size_t)d2 + hoff;
+  const uint32_t ncell = (uint32_t)u.nrows * s.C;
+  uint32_t cell = fdiv(threadIdx.x, p.div_chunks);
+  uint32_t ch = threadIdx.x - cell * p.chunks;
+  if (cm.Cv == s.C) {
+    // all columns valid: slot index = cell index
+    uint32_t soff = cell * p.slot_stride + ch * 16;
+    uint32_t goff = cell * d2 + ch * 16;
+    const uint32_t ds_lo = p.ld_dcell * p.slot_stride + p.ld_dch * 16, dg_lo = p.ld_dcell * d2 + p.ld_dch * 16;
+    const uint32_t ds_wrap = p.slot_stride - p.chunks * 16, dg_wrap = d2 - p.chunks * 16;
+    while (cell < ncell) {
 #pragma unroll
-      for (int k = 0; k < NIN; ++k) cp_async16(stage + k * p.slot_bytes + soff, in[k] + goff);
-      if (r == 0 && ch == 0) stage_ptr[p.off_vcol + v] = (unsigned char)c;
-    } else {
+      for (int k = 0; k < NIN; ++k) cp_async16(stage + k * p.slot_bytes + soff, in[k] + gbase + goff);
+      cell += p.ld_dcell; ch += p.ld_dch; soff += ds_lo; goff += dg_lo;
+      if (ch >= (uint32_t)p.chunks) { ch -= p.chunks; ++cell; soff += ds_wrap; goff += dg_wrap; }
+    }
+    if (threadIdx.x < (uint32_t)s.C) stage_ptr[p.off_vcol + threadIdx.x] = (unsigned char)threadIdx.x;
+  } else {
+    while (cell < ncell) {
+      const uint32_t r = fdiv(cell, p.div_C);
+      const int c = (int)(cell - r * s.C);
+      const size_t g = gbase + (size_t)cell * d2 + ch * 16;
+      if (cm.valid(c)) {
+        const int v = cm.rank(c);
+        const uint32_t soff = (r * cm.Cv + v) * p.slot_stride + ch * 16;
 #pragma unroll
-      for (int k = 0; k < NOUT; ++k) stg_v4(out[k] + goff, make_uint4(0, 0, 0, 0));
-      if (!BWD && ch == 0) {
-        for (int hl = 0; hl < p.hg; ++hl) LSE_out[((row0 + r) * s.H + u.hgi * p.hg + hl) * s.C + c] = 0.f;
+        for (int k = 0; k < NIN; ++k) cp_async16(stage + k * p.slot_bytes + soff, in[k] + g);
+        if (r == 0 && ch == 0) stage_ptr[p.off_vcol + v] = (unsigned char)c;
+      } else {
+#pragma unroll
+        for (int k = 0; k < NOUT; ++k) stg_v4(out[k] + g, make_uint4(0, 0, 0, 0));
+        if (!BWD && ch == 0) {
+          for (int hl = 0; hl < p.hg; ++hl) LSE_out[((row0 + r) * s.H + u.hgi * p.hg + hl) * s.C + c] = 0.f;
+        }
       }
+      cell += p.ld_dcell; ch += p.ld_dch;
+      if (ch >= (uint32_t)p.chunks) { ch -= p.chunks; ++cell; }
     }
   }
   if (BWD) {
     // saved LSE of the unit's valid (row, head, column) triples -> sL[(r*hg + hl)*Cp + v]
     const uint32_t total2 = (uint32_t)u.nrows * p.hg * s.C;
-    for (uint32_t idx = threadIdx.x; idx < total2; idx += kThreads) {
+    for (uint32_t idx = threadIdx.x; idx < total2; idx += blockDim.x) {
       const uint32_t r = fdiv(idx, p.div_hgC);
       const uint32_t rem = idx - r * p.hg * s.C;
       const uint32_t hl = fdiv(rem, p.div_C);
@@ -210,91 +249,99 @@ __device__ __forceinline__ void issue_stage(const FeatParams& p, const Unit& u, 
   if (threadIdx.x == 0) *reinterpret_cast<int*>(stage_ptr + p.off_cv) = cm.Cv;
 }
 
-// Store a 16 x DH bf16 tile that sits in the warp's staging area to the cells (row r of the unit,
-// compacted columns v0 .. v0+15, head h) of a [B,R,C,H,dh] tensor, as full 16-byte vectors.
+__device__ __forceinline__ void stsm4(uint32_t addr, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
+  asm volatile("stmatrix.sync.aligned.m8n8.x4.shared.b16 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(r0), "r"(r1), "r"(r2),
+               "r"(r3)
+               : "memory");
+}
+
+// Output path of one 16 x DH accumulator tile (C fragments: DH/8 n-tiles, rows g and g+8): scale per
+// row, round to bf16, transpose through the warp's staging tile (stmatrix), and write full 16-byte
+// vectors to the cells (row r of the unit, compacted columns v0..v0+15, head h) of a [B,R,C,H,dh] tensor.
+// `dst_row` points at (table row, column 0, head h); cells of one row are d2 bytes apart.
 template <int DH>
-__device__ __forceinline__ void store_tile(uint32_t stg, unsigned char* dst, const FeatParams& p, const Unit& u, int r,
-                                           int h, int v0, int Cv, const unsigned char* vcol) {
+__device__ __forceinline__ void write_tile(uint32_t stg, const float (&acc)[DH / 8][4], float mul0, float mul1,
+                                           unsigned char* dst_row, uint32_t d2, int v0, int Cv, bool identity,
+                                           const unsigned char* vcol) {
   constexpr int SSTR = DH * 2 + 16, CH = DH / 8;
   const int lane = threadIdx.x & 31;
-  const Shape& s = p.s;
-  const size_t rowcell = ((size_t)u.b * s.R + u.r0 + r) * s.C;
+  {
+    const uint32_t a = stg + ((lane & 7) + ((lane >> 3) & 1) * 8) * SSTR + (lane >> 4) * 16;
 #pragma unroll
-  for (int idx = lane; idx < 16 * CH; idx += 32) {
-    const int row = idx / CH, ch = idx - row * CH;
+    for (int np = 0; np < DH / 16; ++np)
+      stsm4(a + np * 32, pack_bf16(acc[2 * np][0] * mul0, acc[2 * np][1] * mul0),
+            pack_bf16(acc[2 * np][2] * mul1, acc[2 * np][3] * mul1),
+            pack_bf16(acc[2 * np + 1][0] * mul0, acc[2 * np + 1][1] * mul0),
+            pack_bf16(acc[2 * np + 1][2] * mul1, acc[2 * np + 1][3] * mul1));
+  }
+  __syncwarp();
+#pragma unroll
+  for (int it = 0; it < (16 * CH + 31) / 32; ++it) {
+    const int idx = it * 32 + lane;
+    const int row = idx / CH, ch = idx % CH;
     if (v0 + row < Cv) {
-      const int c = vcol[v0 + row];
-      const uint4 val = lds128(stg + row * SSTR + ch * 16);
-      stg_v4(dst + ((rowcell + c) * s.H + h) * (size_t)(DH * 2) + ch * 16, val);
+      const uint32_t c = identity ? (uint32_t)(v0 + row) : (uint32_t)vcol[v0 + row];
+      stg_v4(dst_row + (c * d2 + ch * 16), lds128(stg + row * SSTR + ch * 16));
     }
   }
+  __syncwarp();
 }
 
-// Write an accumulator tile (C fragments of DH/8 n-tiles, rows g and g+8) to the staging area as bf16,
-// scaled per row.
-template <int DH>
-__device__ __forceinline__ void stage_tile(uint32_t stg, const float (&acc)[DH / 8][4], float mul0, float mul1) {
-  constexpr int SSTR = DH * 2 + 16;
-  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-#pragma unroll
-  for (int nt = 0; nt < DH / 8; ++nt) {
-    sts32(stg + g * SSTR + nt * 16 + t * 4, pack_bf16(acc[nt][0] * mul0, acc[nt][1] * mul0));
-    sts32(stg + (g + 8) * SSTR + nt * 16 + t * 4, pack_bf16(acc[nt][2] * mul1, acc[nt][3] * mul1));
-  }
-}
+// What a task needs to know about its stage, its warp and its lane.
+struct TaskCtx {
+  uint32_t stg;              // the warp's staging tile
+  LaneOff lo;
+  uint32_t str, d2;          // slot stride, bytes per cell
+  float c2, scale;           // scale * log2(e), scale
+  int Cv;
+  bool identity;             // all columns valid: slot v is column v
+  const unsigned char* vcol;
+};
 
-// ---- forward task: one warp, 16 query cells (compacted columns v0..v0+15) of one (row, head) -----------
-// sQ/sK/sV: shared byte addresses of the slots at (row r of the unit, column slot 0, this head).
+// ---- forward task: one warp, 16 query cells (slots v0..v0+15) of one (row, head) ------------------------
+// sQ/sK/sV: shared byte addresses of the slots at (row r of the unit, slot 0, this head).
 template <int DH>
-__device__ __forceinline__ void fwd_task(const FeatParams& p, const Unit& u, uint32_t sQ, uint32_t sK, uint32_t sV,
-                                         int r, int h, int v0, int Cv, const unsigned char* vcol, uint32_t stg,
-                                         unsigned char* O, float* __restrict__ LSE) {
+__device__ __forceinline__ void fwd_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, int v0,
+                                         unsigned char* O_row, float* __restrict__ LSE_row) {
   constexpr int KS = DH / 16, NT = DH / 8;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int str = p.slot_stride;
-  const float c2 = p.s.scale * kLog2e;
+  const int Cv = x.Cv;
   uint32_t qa[KS][4];
-  {
-    const uint32_t a = sQ + (v0 + (lane & 15)) * str + (lane >> 4) * 16;
 #pragma unroll
-    for (int ks = 0; ks < KS; ++ks) ldsm4(a + ks * 32, qa[ks]);
-  }
+  for (int ks = 0; ks < KS; ++ks) ldsm4(sQ + v0 * x.str + x.lo.a + ks * 32, qa[ks]);
   float o[NT][4];
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
   float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-  // lane address patterns of the B-fragment loads
-  const uint32_t kb_lane = ((lane & 7) + ((lane >> 4) << 3)) * str + ((lane >> 3) & 1) * 16;  // [n][k] operand
-  const uint32_t vb_lane = ((lane & 7) + (((lane >> 3) & 1) << 3)) * str + (lane >> 4) * 16;  // [k][n] operand
-  for (int k0 = 0; k0 < Cv; k0 += 32) {
-    float sc[4][4];
+  for (int k0 = 0; k0 < Cv; k0 += 16) {
+    float sc[2][4];
+    sc[0][0] = sc[0][1] = sc[0][2] = sc[0][3] = 0.f;
+    sc[1][0] = sc[1][1] = sc[1][2] = sc[1][3] = 0.f;
+    {
+      const uint32_t a = sK + k0 * x.str + x.lo.nb;
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) sc[nt][0] = sc[nt][1] = sc[nt][2] = sc[nt][3] = 0.f;
-#pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (k0 + pr * 16 < Cv) {
-        const uint32_t a = sK + (k0 + pr * 16) * str + kb_lane;
-#pragma unroll
-        for (int ks = 0; ks < KS; ++ks) {
-          uint32_t kb[4];
-          ldsm4(a + ks * 32, kb);
-          mma_bf16(sc[2 * pr], qa[ks], kb[0], kb[1]);
-          mma_bf16(sc[2 * pr + 1], qa[ks], kb[2], kb[3]);
-        }
+      for (int ks = 0; ks < KS; ++ks) {
+        uint32_t kb[4];
+        ldsm4(a + ks * 32, kb);
+        mma_bf16(sc[0], qa[ks], kb[0], kb[1]);
+        mma_bf16(sc[1], qa[ks], kb[2], kb[3]);
       }
     }
-    // scale to log2 units, mask keys >= Cv (padded slots), row maxima of rows g and g+8
-    float mx0 = -INFINITY, mx1 = -INFINITY;
+    // scale to log2 units; keys >= Cv (padded slots) -> -inf
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int key = k0 + nt * 8 + 2 * t + (e & 1);
-        sc[nt][e] = key < Cv ? sc[nt][e] * c2 : -INFINITY;
-      }
-      mx0 = fmaxf(mx0, fmaxf(sc[nt][0], sc[nt][1]));
-      mx1 = fmaxf(mx1, fmaxf(sc[nt][2], sc[nt][3]));
+      for (int e = 0; e < 4; ++e) sc[nt][e] *= x.c2;
+    if (k0 + 16 > Cv) {
+      const int lim = Cv - k0 - 2 * t;   // key offset nt*8 + (e&1) must be < lim
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          if (nt * 8 + (e & 1) >= lim) sc[nt][e] = -INFINITY;
     }
+    float mx0 = fmaxf(fmaxf(sc[0][0], sc[0][1]), fmaxf(sc[1][0], sc[1][1]));
+    float mx1 = fmaxf(fmaxf(sc[0][2], sc[0][3]), fmaxf(sc[1][2], sc[1][3]));
     mx0 = quad_max(mx0);
     mx1 = quad_max(mx1);
     const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: the chunk holds >= 1 valid key
@@ -310,122 +357,50 @@ __device__ __forceinline__ void fwd_task(const FeatParams& p, const Unit& u, uin
     }
     m0 = mn0;
     m1 = mn1;
-    uint32_t pa[2][4];
+    uint32_t pa[4];
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt) {
       const float p0 = fast_exp2(sc[nt][0] - m0), p1 = fast_exp2(sc[nt][1] - m0);
       const float p2 = fast_exp2(sc[nt][2] - m1), p3 = fast_exp2(sc[nt][3] - m1);
       l0 += p0 + p1;
       l1 += p2 + p3;
-      pa[nt >> 1][(nt & 1) * 2] = pack_bf16(p0, p1);
-      pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
+      pa[nt * 2] = pack_bf16(p0, p1);
+      pa[nt * 2 + 1] = pack_bf16(p2, p3);
     }
+    {
+      const uint32_t a = sV + k0 * x.str + x.lo.tb;
 #pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (k0 + pr * 16 < Cv) {
-        const uint32_t a = sV + (k0 + pr * 16) * str + vb_lane;
-#pragma unroll
-        for (int np = 0; np < NT / 2; ++np) {
-          uint32_t vb[4];
-          ldsm4t(a + np * 32, vb);
-          mma_bf16(o[2 * np], pa[pr], vb[0], vb[1]);
-          mma_bf16(o[2 * np + 1], pa[pr], vb[2], vb[3]);
-        }
+      for (int np = 0; np < NT / 2; ++np) {
+        uint32_t vb[4];
+        ldsm4t(a + np * 32, vb);
+        mma_bf16(o[2 * np], pa, vb[0], vb[1]);
+        mma_bf16(o[2 * np + 1], pa, vb[2], vb[3]);
       }
     }
   }
   l0 = quad_sum(l0);
   l1 = quad_sum(l1);
-  stage_tile<DH>(stg, o, 1.f / l0, 1.f / l1);
-  __syncwarp();
-  store_tile<DH>(stg, O, p, u, r, h, v0, Cv, vcol);
   if (t == 0) {
-    const Shape& s = p.s;
-    float* lrow = LSE + (((size_t)u.b * s.R + u.r0 + r) * s.H + h) * s.C;
-    if (v0 + g < Cv) lrow[vcol[v0 + g]] = (m0 + log2f(l0)) * kLn2;
-    if (v0 + g + 8 < Cv) lrow[vcol[v0 + g + 8]] = (m1 + log2f(l1)) * kLn2;
+    if (v0 + g < Cv) LSE_row[x.identity ? v0 + g : x.vcol[v0 + g]] = (m0 + log2f(l0)) * kLn2;
+    if (v0 + g + 8 < Cv) LSE_row[x.identity ? v0 + g + 8 : x.vcol[v0 + g + 8]] = (m1 + log2f(l1)) * kLn2;
   }
-  __syncwarp();
-}
-
-template <int DH, int NSTAGE>
-__global__ void __launch_bounds__(kThreads) feature_fwd_mma_kernel(const __grid_constant__ FeatParams p,
-                                                                   const unsigned char* __restrict__ Q,
-                                                                   const unsigned char* __restrict__ K,
-                                                                   const unsigned char* __restrict__ V,
-                                                                   unsigned char* __restrict__ O,
-                                                                   float* __restrict__ LSE, uint32_t smem_total) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  for (uint32_t i = threadIdx.x * 16; i < smem_total; i += kThreads * 16)
-    *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
-  __syncthreads();
-  const uint32_t sbase = smem_addr(smem);
-  const int warp = threadIdx.x >> 5;
-  const uint32_t stg = sbase + warp * 16 * (DH * 2 + 16);
-  const unsigned char* const in[3] = {Q, K, V};
-  unsigned char* const out[1] = {O};
-
-  Unit ld, cu;
-  ld.init(p);
-  cu = ld;
-#pragma unroll
-  for (int q = 0; q < NSTAGE - 1; ++q) {
-    if (ld.ok(p)) {
-      issue_stage<3, 1, false>(p, ld, sbase + p.stage0 + q * p.stage_bytes, smem + p.stage0 + q * p.stage_bytes, in, out,
-                               LSE, nullptr);
-      ld.next(p);
-    }
-    cp_async_commit();
-  }
-  for (uint32_t q = 0; cu.ok(p); ++q, cu.next(p)) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();   // stage q has landed for everyone; everyone is done with stage q-1
-    {
-      const uint32_t nb = (q + NSTAGE - 1) % NSTAGE;
-      if (ld.ok(p)) {
-        issue_stage<3, 1, false>(p, ld, sbase + p.stage0 + nb * p.stage_bytes, smem + p.stage0 + nb * p.stage_bytes, in,
-                                 out, LSE, nullptr);
-        ld.next(p);
-      }
-      cp_async_commit();
-    }
-    const uint32_t buf = q % NSTAGE;
-    const uint32_t stage = sbase + p.stage0 + buf * p.stage_bytes;
-    const unsigned char* sp = smem + p.stage0 + buf * p.stage_bytes;
-    const int Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
-    const unsigned char* vcol = sp + p.off_vcol;
-    const int MT = (Cv + 15) >> 4;
-    const int ntask = cu.nrows * p.hg * MT;
-    for (int task = warp; task < ntask; task += kWarps) {
-      const int mt = task % MT, rest = task / MT;
-      const int hl = rest % p.hg, r = rest / p.hg;
-      const uint32_t off = (uint32_t)(r * p.Cp) * p.slot_stride + hl * DH * 2;
-      fwd_task<DH>(p, cu, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off, r,
-                   cu.hgi * p.hg + hl, mt * 16, Cv, vcol, stg, O, LSE);
-    }
-  }
-  cp_async_wait<0>();
+  write_tile<DH>(x.stg, o, 1.f / l0, 1.f / l1, O_row, x.d2, v0, Cv, x.identity, x.vcol);
 }
 
 // ---- backward, key-stationary task: 16 key cells (slots j0..j0+15) of one (row, head) -> dV, dK -----------
 // sL / sD: this (row, head)'s lse*log2e and D vectors, indexed by column slot.
 template <int DH>
-__device__ __forceinline__ void bwd_key_task(const FeatParams& p, const Unit& u, uint32_t sQ, uint32_t sK, uint32_t sV,
-                                             uint32_t sG, const float* sL, const float* sD, int r, int h, int j0,
-                                             int Cv, const unsigned char* vcol, uint32_t stg, unsigned char* dK,
-                                             unsigned char* dV) {
+__device__ __forceinline__ void bwd_key_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, uint32_t sG,
+                                             const float* sL, const float* sD, int j0, unsigned char* dK_row,
+                                             unsigned char* dV_row) {
   constexpr int KS = DH / 16, NT = DH / 8;
   const int lane = threadIdx.x & 31, t = lane & 3;
-  const int str = p.slot_stride;
-  const float c2 = p.s.scale * kLog2e;
+  const int Cv = x.Cv;
   uint32_t ka[KS][4], va[KS][4];
-  {
-    const uint32_t off = (j0 + (lane & 15)) * str + (lane >> 4) * 16;
 #pragma unroll
-    for (int ks = 0; ks < KS; ++ks) {
-      ldsm4(sK + off + ks * 32, ka[ks]);
-      ldsm4(sV + off + ks * 32, va[ks]);
-    }
+  for (int ks = 0; ks < KS; ++ks) {
+    ldsm4(sK + j0 * x.str + x.lo.a + ks * 32, ka[ks]);
+    ldsm4(sV + j0 * x.str + x.lo.a + ks * 32, va[ks]);
   }
   float dv[NT][4], dk[NT][4];
 #pragma unroll
@@ -433,211 +408,277 @@ __device__ __forceinline__ void bwd_key_task(const FeatParams& p, const Unit& u,
     dv[nt][0] = dv[nt][1] = dv[nt][2] = dv[nt][3] = 0.f;
     dk[nt][0] = dk[nt][1] = dk[nt][2] = dk[nt][3] = 0.f;
   }
-  const uint32_t nb_lane = ((lane & 7) + ((lane >> 4) << 3)) * str + ((lane >> 3) & 1) * 16;  // [n][k] operand
-  const uint32_t tb_lane = ((lane & 7) + (((lane >> 3) & 1) << 3)) * str + (lane >> 4) * 16;  // [k][n] operand
-  for (int i0 = 0; i0 < Cv; i0 += 32) {
-    float st[4][4], dp[4][4];
+  for (int i0 = 0; i0 < Cv; i0 += 16) {
+    float st[2][4], dp[2][4];
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt) {
       st[nt][0] = st[nt][1] = st[nt][2] = st[nt][3] = 0.f;
       dp[nt][0] = dp[nt][1] = dp[nt][2] = dp[nt][3] = 0.f;
     }
+    {
+      const uint32_t off = i0 * x.str + x.lo.nb;
 #pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (i0 + pr * 16 < Cv) {
-        const uint32_t off = (i0 + pr * 16) * str + nb_lane;
-#pragma unroll
-        for (int ks = 0; ks < KS; ++ks) {
-          uint32_t b[4];
-          ldsm4(sQ + off + ks * 32, b);
-          mma_bf16(st[2 * pr], ka[ks], b[0], b[1]);
-          mma_bf16(st[2 * pr + 1], ka[ks], b[2], b[3]);
-          ldsm4(sG + off + ks * 32, b);
-          mma_bf16(dp[2 * pr], va[ks], b[0], b[1]);
-          mma_bf16(dp[2 * pr + 1], va[ks], b[2], b[3]);
-        }
+      for (int ks = 0; ks < KS; ++ks) {
+        uint32_t b[4];
+        ldsm4(sQ + off + ks * 32, b);
+        mma_bf16(st[0], ka[ks], b[0], b[1]);
+        mma_bf16(st[1], ka[ks], b[2], b[3]);
+        ldsm4(sG + off + ks * 32, b);
+        mma_bf16(dp[0], va[ks], b[0], b[1]);
+        mma_bf16(dp[1], va[ks], b[2], b[3]);
       }
     }
     // P^T[j][i] = exp2(S^T c2 - lse2_i), dS^T = P^T (dP^T - D_i); queries i >= Cv (padded slots) -> 0
-    uint32_t pa[2][4], da[2][4];
+    uint32_t pa[4], da[4];
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt) {
       const int i = i0 + nt * 8 + 2 * t;
       const float2 L = *reinterpret_cast<const float2*>(sL + i);
       const float2 D = *reinterpret_cast<const float2*>(sD + i);
       const bool ok0 = i < Cv, ok1 = i + 1 < Cv;
-      const float p0 = ok0 ? fast_exp2(fmaf(st[nt][0], c2, -L.x)) : 0.f;
-      const float p1 = ok1 ? fast_exp2(fmaf(st[nt][1], c2, -L.y)) : 0.f;
-      const float p2 = ok0 ? fast_exp2(fmaf(st[nt][2], c2, -L.x)) : 0.f;
-      const float p3 = ok1 ? fast_exp2(fmaf(st[nt][3], c2, -L.y)) : 0.f;
-      pa[nt >> 1][(nt & 1) * 2] = pack_bf16(p0, p1);
-      pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
-      da[nt >> 1][(nt & 1) * 2] = pack_bf16(p0 * (dp[nt][0] - D.x), p1 * (dp[nt][1] - D.y));
-      da[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2 * (dp[nt][2] - D.x), p3 * (dp[nt][3] - D.y));
+      const float p0 = ok0 ? fast_exp2(fmaf(st[nt][0], x.c2, -L.x)) : 0.f;
+      const float p1 = ok1 ? fast_exp2(fmaf(st[nt][1], x.c2, -L.y)) : 0.f;
+      const float p2 = ok0 ? fast_exp2(fmaf(st[nt][2], x.c2, -L.x)) : 0.f;
+      const float p3 = ok1 ? fast_exp2(fmaf(st[nt][3], x.c2, -L.y)) : 0.f;
+      pa[nt * 2] = pack_bf16(p0, p1);
+      pa[nt * 2 + 1] = pack_bf16(p2, p3);
+      da[nt * 2] = pack_bf16(p0 * (dp[nt][0] - D.x), p1 * (dp[nt][1] - D.y));
+      da[nt * 2 + 1] = pack_bf16(p2 * (dp[nt][2] - D.x), p3 * (dp[nt][3] - D.y));
     }
+    {
+      const uint32_t off = i0 * x.str + x.lo.tb;
 #pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (i0 + pr * 16 < Cv) {
-        const uint32_t off = (i0 + pr * 16) * str + tb_lane;
-#pragma unroll
-        for (int np = 0; np < NT / 2; ++np) {
-          uint32_t b[4];
-          ldsm4t(sG + off + np * 32, b);
-          mma_bf16(dv[2 * np], pa[pr], b[0], b[1]);
-          mma_bf16(dv[2 * np + 1], pa[pr], b[2], b[3]);
-          ldsm4t(sQ + off + np * 32, b);
-          mma_bf16(dk[2 * np], da[pr], b[0], b[1]);
-          mma_bf16(dk[2 * np + 1], da[pr], b[2], b[3]);
-        }
+      for (int np = 0; np < NT / 2; ++np) {
+        uint32_t b[4];
+        ldsm4t(sG + off + np * 32, b);
+        mma_bf16(dv[2 * np], pa, b[0], b[1]);
+        mma_bf16(dv[2 * np + 1], pa, b[2], b[3]);
+        ldsm4t(sQ + off + np * 32, b);
+        mma_bf16(dk[2 * np], da, b[0], b[1]);
+        mma_bf16(dk[2 * np + 1], da, b[2], b[3]);
       }
     }
   }
-  stage_tile<DH>(stg, dv, 1.f, 1.f);
-  __syncwarp();
-  store_tile<DH>(stg, dV, p, u, r, h, j0, Cv, vcol);
-  __syncwarp();
-  stage_tile<DH>(stg, dk, p.s.scale, p.s.scale);
-  __syncwarp();
-  store_tile<DH>(stg, dK, p, u, r, h, j0, Cv, vcol);
-  __syncwarp();
+  write_tile<DH>(x.stg, dv, 1.f, 1.f, dV_row, x.d2, j0, Cv, x.identity, x.vcol);
+  write_tile<DH>(x.stg, dk, x.scale, x.scale, dK_row, x.d2, j0, Cv, x.identity, x.vcol);
 }
 
 // ---- backward, query-stationary task: 16 query cells (slots i0..i0+15) of one (row, head) -> dQ -----------
 template <int DH>
-__device__ __forceinline__ void bwd_query_task(const FeatParams& p, const Unit& u, uint32_t sQ, uint32_t sK,
-                                               uint32_t sV, uint32_t sG, const float* sL, const float* sD, int r, int h,
-                                               int i0, int Cv, const unsigned char* vcol, uint32_t stg,
-                                               unsigned char* dQ) {
+__device__ __forceinline__ void bwd_query_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, uint32_t sG,
+                                               const float* sL, const float* sD, int i0, unsigned char* dQ_row) {
   constexpr int KS = DH / 16, NT = DH / 8;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int str = p.slot_stride;
-  const float c2 = p.s.scale * kLog2e;
+  const int Cv = x.Cv;
   uint32_t qa[KS][4], ga[KS][4];
-  {
-    const uint32_t off = (i0 + (lane & 15)) * str + (lane >> 4) * 16;
 #pragma unroll
-    for (int ks = 0; ks < KS; ++ks) {
-      ldsm4(sQ + off + ks * 32, qa[ks]);
-      ldsm4(sG + off + ks * 32, ga[ks]);
-    }
+  for (int ks = 0; ks < KS; ++ks) {
+    ldsm4(sQ + i0 * x.str + x.lo.a + ks * 32, qa[ks]);
+    ldsm4(sG + i0 * x.str + x.lo.a + ks * 32, ga[ks]);
   }
   // rows g and g+8 of the tile; padded rows read stale (finite) statistics and are never stored
   const float L0 = sL[i0 + g], L1 = sL[i0 + g + 8], D0 = sD[i0 + g], D1 = sD[i0 + g + 8];
   float dq[NT][4];
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) dq[nt][0] = dq[nt][1] = dq[nt][2] = dq[nt][3] = 0.f;
-  const uint32_t nb_lane = ((lane & 7) + ((lane >> 4) << 3)) * str + ((lane >> 3) & 1) * 16;
-  const uint32_t tb_lane = ((lane & 7) + (((lane >> 3) & 1) << 3)) * str + (lane >> 4) * 16;
-  for (int k0 = 0; k0 < Cv; k0 += 32) {
-    float sc[4][4], dp[4][4];
+  for (int k0 = 0; k0 < Cv; k0 += 16) {
+    float sc[2][4], dp[2][4];
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt) {
       sc[nt][0] = sc[nt][1] = sc[nt][2] = sc[nt][3] = 0.f;
       dp[nt][0] = dp[nt][1] = dp[nt][2] = dp[nt][3] = 0.f;
     }
+    {
+      const uint32_t off = k0 * x.str + x.lo.nb;
 #pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (k0 + pr * 16 < Cv) {
-        const uint32_t off = (k0 + pr * 16) * str + nb_lane;
-#pragma unroll
-        for (int ks = 0; ks < KS; ++ks) {
-          uint32_t b[4];
-          ldsm4(sK + off + ks * 32, b);
-          mma_bf16(sc[2 * pr], qa[ks], b[0], b[1]);
-          mma_bf16(sc[2 * pr + 1], qa[ks], b[2], b[3]);
-          ldsm4(sV + off + ks * 32, b);
-          mma_bf16(dp[2 * pr], ga[ks], b[0], b[1]);
-          mma_bf16(dp[2 * pr + 1], ga[ks], b[2], b[3]);
-        }
+      for (int ks = 0; ks < KS; ++ks) {
+        uint32_t b[4];
+        ldsm4(sK + off + ks * 32, b);
+        mma_bf16(sc[0], qa[ks], b[0], b[1]);
+        mma_bf16(sc[1], qa[ks], b[2], b[3]);
+        ldsm4(sV + off + ks * 32, b);
+        mma_bf16(dp[0], ga[ks], b[0], b[1]);
+        mma_bf16(dp[1], ga[ks], b[2], b[3]);
       }
     }
-    uint32_t da[2][4];
+    uint32_t da[4];
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
+    for (int nt = 0; nt < 2; ++nt) {
       const int key = k0 + nt * 8 + 2 * t;
       const bool ok0 = key < Cv, ok1 = key + 1 < Cv;   // keys in padded slots: P = 0 exactly
-      const float p0 = ok0 ? fast_exp2(fmaf(sc[nt][0], c2, -L0)) : 0.f;
-      const float p1 = ok1 ? fast_exp2(fmaf(sc[nt][1], c2, -L0)) : 0.f;
-      const float p2 = ok0 ? fast_exp2(fmaf(sc[nt][2], c2, -L1)) : 0.f;
-      const float p3 = ok1 ? fast_exp2(fmaf(sc[nt][3], c2, -L1)) : 0.f;
-      da[nt >> 1][(nt & 1) * 2] = pack_bf16(p0 * (dp[nt][0] - D0), p1 * (dp[nt][1] - D0));
-      da[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2 * (dp[nt][2] - D1), p3 * (dp[nt][3] - D1));
+      const float p0 = ok0 ? fast_exp2(fmaf(sc[nt][0], x.c2, -L0)) : 0.f;
+      const float p1 = ok1 ? fast_exp2(fmaf(sc[nt][1], x.c2, -L0)) : 0.f;
+      const float p2 = ok0 ? fast_exp2(fmaf(sc[nt][2], x.c2, -L1)) : 0.f;
+      const float p3 = ok1 ? fast_exp2(fmaf(sc[nt][3], x.c2, -L1)) : 0.f;
+      da[nt * 2] = pack_bf16(p0 * (dp[nt][0] - D0), p1 * (dp[nt][1] - D0));
+      da[nt * 2 + 1] = pack_bf16(p2 * (dp[nt][2] - D1), p3 * (dp[nt][3] - D1));
     }
+    {
+      const uint32_t off = k0 * x.str + x.lo.tb;
 #pragma unroll
-    for (int pr = 0; pr < 2; ++pr) {
-      if (k0 + pr * 16 < Cv) {
-        const uint32_t off = (k0 + pr * 16) * str + tb_lane;
-#pragma unroll
-        for (int np = 0; np < NT / 2; ++np) {
-          uint32_t b[4];
-          ldsm4t(sK + off + np * 32, b);
-          mma_bf16(dq[2 * np], da[pr], b[0], b[1]);
-          mma_bf16(dq[2 * np + 1], da[pr], b[2], b[3]);
-        }
+      for (int np = 0; np < NT / 2; ++np) {
+        uint32_t b[4];
+        ldsm4t(sK + off + np * 32, b);
+        mma_bf16(dq[2 * np], da, b[0], b[1]);
+        mma_bf16(dq[2 * np + 1], da, b[2], b[3]);
       }
     }
   }
-  stage_tile<DH>(stg, dq, p.s.scale, p.s.scale);
-  __syncwarp();
-  store_tile<DH>(stg, dQ, p, u, r, h, i0, Cv, vcol);
-  __syncwarp();
+  write_tile<DH>(x.stg, dq, x.scale, x.scale, dQ_row, x.d2, i0, Cv, x.identity, x.vcol);
+}
+
+// ---- kernels -------------------------------------------------------------------------------------------------
+// Task walker of one warp inside a stage: tasks (tile mt, head hl, row r), mt fastest, strided by the
+// warp count; advanced with carries instead of divisions.
+struct TaskIt {
+  int mt, hl, r;
+  __device__ __forceinline__ void carry(int MT, int hg) {
+    while (mt >= MT) { mt -= MT; ++hl; }
+    while (hl >= hg) { hl -= hg; ++r; }
+  }
+};
+
+__device__ __forceinline__ void zero_smem(unsigned char* smem, uint32_t smem_total) {
+  for (uint32_t i = threadIdx.x * 16; i < smem_total; i += blockDim.x * 16)
+    *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
+  __syncthreads();
 }
 
 template <int DH, int NSTAGE>
-__global__ void __launch_bounds__(kThreads) feature_bwd_mma_kernel(
-    const __grid_constant__ FeatParams p, const unsigned char* __restrict__ Q, const unsigned char* __restrict__ K,
-    const unsigned char* __restrict__ V, const unsigned char* __restrict__ O, const unsigned char* __restrict__ dO,
-    const float* __restrict__ LSE, unsigned char* __restrict__ dQ, unsigned char* __restrict__ dK,
-    unsigned char* __restrict__ dV, uint32_t smem_total) {
+__global__ void __launch_bounds__(kMaxWarps * 32) feature_fwd_mma_kernel(const __grid_constant__ FeatParams p,
+                                                                         const unsigned char* __restrict__ Q,
+                                                                         const unsigned char* __restrict__ K,
+                                                                         const unsigned char* __restrict__ V,
+                                                                         unsigned char* __restrict__ O,
+                                                                         float* __restrict__ LSE, uint32_t smem_total) {
   extern __shared__ __align__(16) unsigned char smem[];
-  for (uint32_t i = threadIdx.x * 16; i < smem_total; i += kThreads * 16)
-    *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
-  __syncthreads();
+  zero_smem(smem, smem_total);
   const uint32_t sbase = smem_addr(smem);
-  const int warp = threadIdx.x >> 5;
-  const uint32_t stg = sbase + warp * 16 * (DH * 2 + 16);
-  // slot order: Q, K, V, dO, O
-  const unsigned char* const in[5] = {Q, K, V, dO, O};
-  unsigned char* const out[3] = {dQ, dK, dV};
+  const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  const unsigned char* const in[3] = {Q, K, V};
+  unsigned char* const out[1] = {O};
+  const Shape& s = p.s;
+  TaskCtx x;
+  x.stg = sbase + warp * 16 * (DH * 2 + 16);
+  x.lo.init(p.slot_stride);
+  x.str = p.slot_stride;
+  x.d2 = s.H * DH * 2;
+  x.c2 = s.scale * kLog2e;
+  x.scale = s.scale;
 
   Unit ld, cu;
+  ColMask cm;
   ld.init(p);
   cu = ld;
 #pragma unroll
   for (int q = 0; q < NSTAGE - 1; ++q) {
     if (ld.ok(p)) {
-      issue_stage<5, 3, true>(p, ld, sbase + p.stage0 + q * p.stage_bytes, smem + p.stage0 + q * p.stage_bytes, in, out,
-                              nullptr, LSE);
+      issue_stage<3, 1, false>(p, ld, cm, sbase + p.stage0 + q * p.stage_bytes, smem + p.stage0 + q * p.stage_bytes, in,
+                               out, LSE, nullptr);
       ld.next(p);
     }
     cp_async_commit();
   }
-  for (uint32_t q = 0; cu.ok(p); ++q, cu.next(p)) {
+  uint32_t buf = 0;
+  for (; cu.ok(p); cu.next(p)) {
     cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
+    __syncthreads();   // stage `buf` has landed for everyone; everyone is done with the previous stage
     {
-      const uint32_t nb = (q + NSTAGE - 1) % NSTAGE;
+      const uint32_t nb = buf == 0 ? NSTAGE - 1 : buf - 1;
       if (ld.ok(p)) {
-        issue_stage<5, 3, true>(p, ld, sbase + p.stage0 + nb * p.stage_bytes, smem + p.stage0 + nb * p.stage_bytes, in,
-                                out, nullptr, LSE);
+        issue_stage<3, 1, false>(p, ld, cm, sbase + p.stage0 + nb * p.stage_bytes, smem + p.stage0 + nb * p.stage_bytes,
+                                 in, out, LSE, nullptr);
         ld.next(p);
       }
       cp_async_commit();
     }
-    const uint32_t buf = q % NSTAGE;
+    const uint32_t stage = sbase + p.stage0 + buf * p.stage_bytes;
+    const unsigned char* sp = smem + p.stage0 + buf * p.stage_bytes;
+    x.Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
+    x.vcol = sp + p.off_vcol;
+    x.identity = x.Cv == s.C;
+    const int MT = (x.Cv + 15) >> 4;
+    const size_t row0 = (size_t)cu.b * s.R + cu.r0;
+    TaskIt it{warp, 0, 0};
+    if (MT > 0) {
+      for (it.carry(MT, p.hg); it.r < cu.nrows; it.mt += nwarps, it.carry(MT, p.hg)) {
+        const uint32_t off = (uint32_t)(it.r * x.Cv) * p.slot_stride + it.hl * DH * 2;
+        const int h = cu.hgi * p.hg + it.hl;
+        fwd_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off, it.mt * 16,
+                     O + (row0 + it.r) * s.C * x.d2 + h * DH * 2, LSE + ((row0 + it.r) * s.H + h) * s.C);
+      }
+    }
+    buf = buf + 1 == NSTAGE ? 0 : buf + 1;
+  }
+  cp_async_wait<0>();
+}
+
+template <int DH, int NSTAGE>
+__global__ void __launch_bounds__(kMaxWarps * 32) feature_bwd_mma_kernel(
+    const __grid_constant__ FeatParams p, const unsigned char* __restrict__ Q, const unsigned char* __restrict__ K,
+    const unsigned char* __restrict__ V, const unsigned char* __restrict__ O, const unsigned char* __restrict__ dO,
+    const float* __restrict__ LSE, unsigned char* __restrict__ dQ, unsigned char* __restrict__ dK,
+    unsigned char* __restrict__ dV, uint32_t smem_total) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  zero_smem(smem, smem_total);
+  const uint32_t sbase = smem_addr(smem);
+  const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  // slot order: Q, K, V, dO, O
+  const unsigned char* const in[5] = {Q, K, V, dO, O};
+  unsigned char* const out[3] = {dQ, dK, dV};
+  const Shape& s = p.s;
+  TaskCtx x;
+  x.stg = sbase + warp * 16 * (DH * 2 + 16);
+  x.lo.init(p.slot_stride);
+  x.str = p.slot_stride;
+  x.d2 = s.H * DH * 2;
+  x.c2 = s.scale * kLog2e;
+  x.scale = s.scale;
+
+  Unit ld, cu;
+  ColMask cm;
+  ld.init(p);
+  cu = ld;
+#pragma unroll
+  for (int q = 0; q < NSTAGE - 1; ++q) {
+    if (ld.ok(p)) {
+      issue_stage<5, 3, true>(p, ld, cm, sbase + p.stage0 + q * p.stage_bytes, smem + p.stage0 + q * p.stage_bytes, in,
+                              out, nullptr, LSE);
+      ld.next(p);
+    }
+    cp_async_commit();
+  }
+  uint32_t buf = 0;
+  for (; cu.ok(p); cu.next(p)) {
+    cp_async_wait<NSTAGE - 2>();
+    __syncthreads();
+    {
+      const uint32_t nb = buf == 0 ? NSTAGE - 1 : buf - 1;
+      if (ld.ok(p)) {
+        issue_stage<5, 3, true>(p, ld, cm, sbase + p.stage0 + nb * p.stage_bytes, smem + p.stage0 + nb * p.stage_bytes,
+                                in, out, nullptr, LSE);
+        ld.next(p);
+      }
+      cp_async_commit();
+    }
     const uint32_t stage = sbase + p.stage0 + buf * p.stage_bytes;
     unsigned char* sp = smem + p.stage0 + buf * p.stage_bytes;
-    const int Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
-    const unsigned char* vcol = sp + p.off_vcol;
+    x.Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
+    x.vcol = sp + p.off_vcol;
+    x.identity = x.Cv == s.C;
+    const int Cv = x.Cv;
     float* sL = reinterpret_cast<float*>(sp + p.off_lse);
     float* sD = reinterpret_cast<float*>(sp + p.off_D);
-    // D[r][hl][v] = sum_k dO O over the head's dh elements; LSE -> log2 units
-    {
-      const int n = cu.nrows * p.hg * Cv;
-      for (int idx = threadIdx.x; idx < n; idx += kThreads) {
-        const int v = idx % Cv, rest = idx / Cv;
-        const int hl = rest % p.hg, r = rest / p.hg;
-        const uint32_t off = (uint32_t)(r * p.Cp + v) * p.slot_stride + hl * DH * 2;
+    // D[r][hl][v] = sum_k dO O over the head's dh elements; LSE -> log2 units.  Thread <-> (r, hl, v).
+    if (Cv > 0) {
+      int v = threadIdx.x, rh = 0;
+      const int nrh = cu.nrows * p.hg;
+      while (true) {
+        while (v >= Cv) { v -= Cv; ++rh; }
+        if (rh >= nrh) break;
+        int r = 0, hl = rh;
+        while (hl >= p.hg) { hl -= p.hg; ++r; }
+        const uint32_t off = (uint32_t)(r * Cv + v) * p.slot_stride + hl * DH * 2;
         float acc = 0.f;
 #pragma unroll
         for (int k = 0; k < DH / 8; ++k) {
@@ -647,30 +688,39 @@ __global__ void __launch_bounds__(kThreads) feature_bwd_mma_kernel(
 #pragma unroll
           for (int e = 0; e < 8; ++e) acc = fmaf(a[e], g[e], acc);
         }
-        const int si = (r * p.hg + hl) * p.Cp + v;
+        const int si = rh * p.Cp + v;
         sD[si] = acc;
         sL[si] *= kLog2e;
+        v += blockDim.x;
       }
     }
     __syncthreads();
     const int MT = (Cv + 15) >> 4;
-    const int nhalf = cu.nrows * p.hg * MT;
-    for (int task = warp; task < 2 * nhalf; task += kWarps) {
-      const bool key_task = task < nhalf;
-      const int tk = key_task ? task : task - nhalf;
-      const int mt = tk % MT, rest = tk / MT;
-      const int hl = rest % p.hg, r = rest / p.hg;
-      const uint32_t off = (uint32_t)(r * p.Cp) * p.slot_stride + hl * DH * 2;
-      const float* L = sL + (r * p.hg + hl) * p.Cp;
-      const float* D = sD + (r * p.hg + hl) * p.Cp;
-      const int h = cu.hgi * p.hg + hl;
+    const size_t rowcell0 = ((size_t)cu.b * s.R + cu.r0) * s.C;
+    // tasks 0 .. nrows*hg*MT-1: key-stationary; the same count again: query-stationary
+    TaskIt it{warp, 0, 0};
+    bool key_task = true;
+    while (MT > 0) {
+      it.carry(MT, p.hg);
+      if (it.r >= cu.nrows) {
+        if (!key_task) break;
+        key_task = false;
+        it.r -= cu.nrows;
+        continue;
+      }
+      const uint32_t off = (uint32_t)(it.r * Cv) * p.slot_stride + it.hl * DH * 2;
+      const float* L = sL + (it.r * p.hg + it.hl) * p.Cp;
+      const float* D = sD + (it.r * p.hg + it.hl) * p.Cp;
+      const size_t goff = (rowcell0 + (size_t)it.r * s.C) * x.d2 + (cu.hgi * p.hg + it.hl) * DH * 2;
       if (key_task)
-        bwd_key_task<DH>(p, cu, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
-                         stage + 3 * p.slot_bytes + off, L, D, r, h, mt * 16, Cv, vcol, stg, dK, dV);
+        bwd_key_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
+                         stage + 3 * p.slot_bytes + off, L, D, it.mt * 16, dK + goff, dV + goff);
       else
-        bwd_query_task<DH>(p, cu, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
-                           stage + 3 * p.slot_bytes + off, L, D, r, h, mt * 16, Cv, vcol, stg, dQ);
+        bwd_query_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
+                           stage + 3 * p.slot_bytes + off, L, D, it.mt * 16, dQ + goff);
+      it.mt += nwarps;
     }
+    buf = buf + 1 == NSTAGE ? 0 : buf + 1;
   }
   cp_async_wait<0>();
 }
@@ -684,38 +734,49 @@ int env_int(const char* name, int dflt) {
 
 constexpr size_t kSmemPerSM = 227 * 1024;
 
-// Picks heads-per-unit, rows-per-unit and ring depth: a stage of roughly 16-48 KB (enough bytes in
-// flight per SM to cover HBM latency with 2-3 CTAs per SM), at least ~3 tasks per warp per stage.
-FeatParams make_plan(const Shape& s, bool bwd, size_t* smem_total, int* ctas_per_sm) {
-  FeatParams p{};
+struct Plan {
+  FeatParams p;
+  size_t smem;
+  int warps, ctas_per_sm;
+};
+
+// Picks heads-per-unit, rows-per-unit, warps per CTA and ring depth.
+Plan make_plan(const Shape& s, bool bwd) {
+  Plan pl{};
+  FeatParams& p = pl.p;
   p.s = s;
   const int nslot = bwd ? 5 : 3;
   p.Cp = (s.C + 15) / 16 * 16;
   auto stage_bytes = [&](int hg, int rows) {
-    size_t slot = (size_t)rows * p.Cp * (hg * s.dh * 2 + 16);
-    size_t b = nslot * slot;
+    const size_t stride = (size_t)hg * s.dh * 2 + 16;
+    size_t b = nslot * (size_t)rows * s.C * stride + 16 * stride;   // slots + read slack after the last one
     if (bwd) b += (size_t)2 * rows * hg * p.Cp * 4;
-    return b + 128 /* vcol */ + 16 /* Cv */ + 256 /* slack for reads of padded statistics */;
+    return b + 256 + 128 /* vcol */ + 16 /* Cv */;
   };
-  const size_t target = 40 * 1024;
+  const size_t target = (size_t)env_int("TABATTN_FEAT_STAGE_KB", 32) * 1024;
   int hg = s.H;
   while (hg > 1 && stage_bytes(hg, 1) > target) {
     int nh = hg - 1;
     while (nh > 1 && (s.H % nh != 0)) --nh;
     hg = nh;
   }
+  hg = env_int("TABATTN_FEAT_HG", hg);
   const int MT = (s.C + 15) / 16;
   const int per_row_tasks = hg * MT * (bwd ? 2 : 1);
+  int warps = 4;
+  {
+    const int cand[] = {4, 6, 8, 3, 5, 7};
+    for (int c : cand)
+      if (per_row_tasks % c == 0) { warps = c; break; }
+  }
+  warps = env_int("TABATTN_FEAT_WARPS", warps);
+  if (warps > kMaxWarps) warps = kMaxWarps;
+  if (warps < 1) warps = 1;
   int rows = 1;
-  while (rows < s.R && rows * per_row_tasks < 3 * kWarps && stage_bytes(hg, rows + 1) <= target) ++rows;
-  hg = env_int("TABATTN_FEAT_HG", hg);
+  while (rows < s.R && rows * per_row_tasks < 2 * warps && stage_bytes(hg, rows + 1) <= target) ++rows;
   rows = env_int("TABATTN_FEAT_ROWS", rows);
-  const size_t stg_bytes = (size_t)kWarps * 16 * (s.dh * 2 + 16);
-  const size_t sb = stage_bytes(hg, rows);
-  int nstage = 3;
-  if (stg_bytes + 3 * sb > 76 * 1024 && stg_bytes + 2 * sb <= kSmemPerSM) nstage = 2;
-  if (stg_bytes + 3 * sb <= 56 * 1024) nstage = 4;
-  nstage = env_int("TABATTN_FEAT_NSTAGE", nstage);
+  const size_t stg_bytes = (size_t)warps * 16 * (s.dh * 2 + 16);
+  int nstage = env_int("TABATTN_FEAT_NSTAGE", 2);
   p.hg = hg;
   p.nhg = s.H / hg;
   p.rows = rows;
@@ -726,8 +787,8 @@ FeatParams make_plan(const Shape& s, bool bwd, size_t* smem_total, int* ctas_per
   p.div_chunks = magic(p.chunks);
   p.div_C = magic(s.C);
   p.div_hgC = magic(hg * s.C);
-  p.slot_bytes = (uint32_t)((size_t)rows * p.Cp * p.slot_stride);
-  uint32_t o = nslot * p.slot_bytes;
+  p.slot_bytes = (uint32_t)((size_t)rows * s.C * p.slot_stride);
+  uint32_t o = nslot * p.slot_bytes + 16 * p.slot_stride;
   p.off_lse = o;
   if (bwd) o += rows * hg * p.Cp * 4;
   p.off_D = o;
@@ -740,10 +801,14 @@ FeatParams make_plan(const Shape& s, bool bwd, size_t* smem_total, int* ctas_per
   p.stage_bytes = o;
   p.stage0 = (uint32_t)stg_bytes;
   p.nstage = nstage;
-  *smem_total = stg_bytes + (size_t)nstage * p.stage_bytes;
-  int per_sm = (int)(kSmemPerSM / (*smem_total + 1024));
-  *ctas_per_sm = per_sm < 1 ? 1 : (per_sm > 4 ? 4 : per_sm);
-  return p;
+  p.ld_dcell = warps * 32 / p.chunks;
+  p.ld_dch = warps * 32 % p.chunks;
+  pl.smem = stg_bytes + (size_t)nstage * p.stage_bytes;
+  pl.warps = warps;
+  int per_sm = (int)(kSmemPerSM / (pl.smem + 1024));
+  per_sm = per_sm < 1 ? 1 : (per_sm > 8 ? 8 : per_sm);
+  pl.ctas_per_sm = env_int("TABATTN_FEAT_CTAS", per_sm);
+  return pl;
 }
 
 }  // namespace
@@ -753,44 +818,46 @@ bool feature_shape_supported(const Shape& s) { return s.C <= 128; }
 namespace {
 
 template <typename Kern, typename... Args>
-cudaError_t launch_persistent(Kern kern, const FeatParams& p, size_t smem, int ctas_per_sm, cudaStream_t stream,
-                              Args... args) {
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+cudaError_t launch_persistent(Kern kern, const Plan& pl, cudaStream_t stream, Args... args) {
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return e;
   int occ = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.warps * 32, pl.smem);
   if (e != cudaSuccess) return e;
   if (occ < 1) return cudaErrorInvalidValue;
-  const int per_sm = occ < ctas_per_sm ? occ : ctas_per_sm;
+  const int per_sm = occ < pl.ctas_per_sm ? occ : pl.ctas_per_sm;
   const long long want = (long long)num_sms() * per_sm;
-  const int grid = (int)(p.n_su < want ? p.n_su : want);
-  kern<<<grid, kThreads, smem, stream>>>(p, args..., (uint32_t)smem);
+  const int grid = (int)(pl.p.n_su < want ? pl.p.n_su : want);
+  if (env_int("TABATTN_FEAT_DEBUG", 0))
+    fprintf(stderr, "feature plan: hg=%d rows=%d warps=%d nstage=%d stage=%u B smem=%zu B occ=%d ctas/sm=%d grid=%d\n",
+            pl.p.hg, pl.p.rows, pl.warps, pl.p.nstage, pl.p.stage_bytes, pl.smem, occ, per_sm, grid);
+  kern<<<grid, pl.warps * 32, pl.smem, stream>>>(pl.p, args..., (uint32_t)pl.smem);
   count_launch();
   return cudaGetLastError();
 }
 
 #define TABATTN_FEAT_DISPATCH(NAME, ...)                                              \
-  switch (s.dh * 10 + p.nstage) {                                                     \
-    case 162: return launch_persistent(NAME<16, 2>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 163: return launch_persistent(NAME<16, 3>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 164: return launch_persistent(NAME<16, 4>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 322: return launch_persistent(NAME<32, 2>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 323: return launch_persistent(NAME<32, 3>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 324: return launch_persistent(NAME<32, 4>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 642: return launch_persistent(NAME<64, 2>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 643: return launch_persistent(NAME<64, 3>, p, smem, per_sm, stream, __VA_ARGS__); \
-    case 644: return launch_persistent(NAME<64, 4>, p, smem, per_sm, stream, __VA_ARGS__); \
+  switch (s.dh * 10 + pl.p.nstage) {                                                  \
+    case 162: return launch_persistent(NAME<16, 2>, pl, stream, __VA_ARGS__);         \
+    case 163: return launch_persistent(NAME<16, 3>, pl, stream, __VA_ARGS__);         \
+    case 322: return launch_persistent(NAME<32, 2>, pl, stream, __VA_ARGS__);         \
+    case 323: return launch_persistent(NAME<32, 3>, pl, stream, __VA_ARGS__);         \
+    case 642: return launch_persistent(NAME<64, 2>, pl, stream, __VA_ARGS__);         \
+    case 643: return launch_persistent(NAME<64, 3>, pl, stream, __VA_ARGS__);         \
     default: return cudaErrorInvalidValue;                                            \
   }
+
+bool plan_ok(const Shape& s, const Plan& pl) {
+  return pl.smem <= kSmemPerSM && pl.p.nstage >= 2 && pl.p.nstage <= 3 && pl.p.hg >= 1 && s.H % pl.p.hg == 0 &&
+         pl.p.rows >= 1;
+}
 
 }  // namespace
 
 cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                cudaStream_t stream) {
-  size_t smem;
-  int per_sm;
-  const FeatParams p = make_plan(s, false, &smem, &per_sm);
-  if (smem > kSmemPerSM || p.nstage < 2 || p.nstage > kMaxStages || s.H % p.hg != 0) return cudaErrorInvalidValue;
+  const Plan pl = make_plan(s, false);
+  if (!plan_ok(s, pl)) return cudaErrorInvalidValue;
   TABATTN_FEAT_DISPATCH(feature_fwd_mma_kernel, (const unsigned char*)Q, (const unsigned char*)K,
                         (const unsigned char*)V, (unsigned char*)O, LSE);
 }
@@ -798,10 +865,8 @@ cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, con
 cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
                                const void* dO, const float* LSE, void* dQ, void* dK, void* dV,
                                cudaStream_t stream) {
-  size_t smem;
-  int per_sm;
-  const FeatParams p = make_plan(s, true, &smem, &per_sm);
-  if (smem > kSmemPerSM || p.nstage < 2 || p.nstage > kMaxStages || s.H % p.hg != 0) return cudaErrorInvalidValue;
+  const Plan pl = make_plan(s, true);
+  if (!plan_ok(s, pl)) return cudaErrorInvalidValue;
   TABATTN_FEAT_DISPATCH(feature_bwd_mma_kernel, (const unsigned char*)Q, (const unsigned char*)K,
                         (const unsigned char*)V, (const unsigned char*)O, (const unsigned char*)dO, LSE,
                         (unsigned char*)dQ, (unsigned char*)dK, (unsigned char*)dV);
