@@ -753,27 +753,22 @@ Plan make_plan(const Shape& s, bool bwd) {
     if (bwd) b += (size_t)2 * rows * hg * p.Cp * 4;
     return b + 256 + 128 /* vcol */ + 16 /* Cv */;
   };
-  const size_t target = (size_t)env_int("TABATTN_FEAT_STAGE_KB", 32) * 1024;
-  int hg = s.H;
+  // Measured on B200 (profiles/r01_feature_mma.md): small CTAs with small stages win -- many CTAs per SM
+  // hide each other's barrier and latency bubbles.  Head groups of 128 contiguous bytes per cell
+  // (one L2 line), 1-2 table rows per stage, 2 warps (C <= 16) or 4 warps per CTA.
+  const size_t target = (size_t)env_int("TABATTN_FEAT_STAGE_KB", 40) * 1024;
+  int hg = 128 / (s.dh * 2);
+  if (hg < 1) hg = 1;
+  while (hg > 1 && s.H % hg != 0) --hg;
   while (hg > 1 && stage_bytes(hg, 1) > target) {
-    int nh = hg - 1;
-    while (nh > 1 && (s.H % nh != 0)) --nh;
-    hg = nh;
+    --hg;
+    while (hg > 1 && s.H % hg != 0) --hg;
   }
   hg = env_int("TABATTN_FEAT_HG", hg);
-  const int MT = (s.C + 15) / 16;
-  const int per_row_tasks = hg * MT * (bwd ? 2 : 1);
-  int warps = 4;
-  {
-    const int cand[] = {4, 6, 8, 3, 5, 7};
-    for (int c : cand)
-      if (per_row_tasks % c == 0) { warps = c; break; }
-  }
-  warps = env_int("TABATTN_FEAT_WARPS", warps);
+  int warps = env_int("TABATTN_FEAT_WARPS", s.C <= 16 ? 2 : 4);
   if (warps > kMaxWarps) warps = kMaxWarps;
   if (warps < 1) warps = 1;
-  int rows = 1;
-  while (rows < s.R && rows * per_row_tasks < 2 * warps && stage_bytes(hg, rows + 1) <= target) ++rows;
+  int rows = (!bwd && s.C <= 32 && s.R >= 2 && stage_bytes(hg, 2) <= target) ? 2 : 1;
   rows = env_int("TABATTN_FEAT_ROWS", rows);
   const size_t stg_bytes = (size_t)warps * 16 * (s.dh * 2 + 16);
   int nstage = env_int("TABATTN_FEAT_NSTAGE", 2);
