@@ -194,6 +194,24 @@ def run_reference(args):
     return 0
 
 
+# ---- multi-rank host logic (replicas only): max over ranks, whole-job value -------------
+def max_over_ranks(ms, world, device=None):
+    """MAX of a per-rank device time over all ranks (identity when world == 1)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(ms_per_step, layers, world):
+    """ms/layer of the whole job: every rank runs one replica of the step, so N ranks finish N layers'
+    worth of work per `layers` layer-times (time-like metric: lower is better)."""
+    return ms_per_step / layers / world
+
+
 # ---- our arm ----------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
@@ -272,11 +290,7 @@ def run_ours(args):
     barrier()
     launches = tab.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = t0.elapsed_time(t1)
-    tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms = float(tt.item())
+    total_ms = max_over_ranks(t0.elapsed_time(t1), world, dev)
     ms_per_step = total_ms / args.steps
     # per-call device times (mean over steps and layers), from events on the launching stream
     names = ["feature_fwd", "item_fwd", "item_bwd", "feature_bwd"]
@@ -304,10 +318,8 @@ def run_ours(args):
                                               out_host, n_train, col_valid, buf, n_train_h)
         b.record(stream)
         barrier()
-        et = torch.tensor([a.elapsed_time(b) / e_steps], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(et, op=dist.ReduceOp.MAX)
-        e2e = {"value": float(et.item()) / world, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        et = max_over_ranks(a.elapsed_time(b) / e_steps, world, dev)
+        e2e = {"value": job_value(et, 1, world), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "note": "one layer per step from pinned host buffers"}
         del host, stage, out_host
 
@@ -352,7 +364,7 @@ def run_ours(args):
         ms_cpu, cores, sample, _ = oracle_sample_ms_per_layer(cfg, budget_s=args.cpu_budget)
         cpu = {"value": ms_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
-    value = ms_per_step / cfg.layers / world
+    value = job_value(ms_per_step, cfg.layers, world)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
