@@ -3,9 +3,9 @@
 // Persistent, warp-specialised kernel; one CTA per SM walks work items (b, c, h, 256 query rows):
 //   warp 8        TMA producer: Q tiles (2 x 128 rows, double-buffered over items) and a ring of K/V
 //                 tiles of the train rows [0, n_train[b]) only
-//   warp 9        MMA issuer (one lane, precomputed descriptors): S_t = Q_t K_j^T (SS, fp32 in TMEM),
-//                 O_t += P_t V_j (A = P in TMEM as bf16)
-//   warp 11       V tail fixer: zeroes the rows >= n_train of a partially valid last key tile
+//   warp 9        issuer of S_t = Q_t K_j^T (SS, fp32 in TMEM) for both query tiles; also zeroes the
+//                 V rows >= n_train of a partially valid last key tile
+//   warp 10 / 11  issuer of O_t += P_t V_j (A = P in TMEM as bf16) for query tile 0 / 1
 //   warps 0-3/4-7 softmax warpgroup of query tile t = 0 / 1: one thread per query row reads its S row
 //                 from TMEM, online softmax in base 2 with lazy rescaling of O, writes P (bf16) back
 //                 to TMEM; epilogue O / l -> bf16, LSE (natural log)
@@ -53,7 +53,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
   const uint32_t sQ = sbase;                               // [QBUF][2][TILE]
   const uint32_t sK = sQ + 2 * Cfg::QBUF * TILE;           // [ST][TILE]
   const uint32_t sV = sK + ST * TILE;                      // [ST][TILE]
-  __shared__ uint64_t bar_q_full[2], bar_q_empty[2], bar_k_full[ST], bar_v_full[ST], bar_v_land[ST], bar_kv_empty[ST];
+  __shared__ uint64_t bar_q_full[2], bar_q_empty[2], bar_k_full[ST], bar_v_full[ST], bar_v_land[ST], bar_k_empty[ST], bar_v_empty[ST];
   __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_pv_done[2];
   __shared__ uint32_t tmem_slot;
 
@@ -72,7 +72,8 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       mbar_init(smem_u32(&bar_k_full[i]), 1);
       mbar_init(smem_u32(&bar_v_full[i]), 1);
       mbar_init(smem_u32(&bar_v_land[i]), 1);
-      mbar_init(smem_u32(&bar_kv_empty[i]), 1);
+      mbar_init(smem_u32(&bar_k_empty[i]), 1);
+      mbar_init(smem_u32(&bar_v_empty[i]), 2);   // both PV issuers
     }
     fence_barrier_init();
   }
@@ -101,121 +102,110 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                         wk.b);
           }
           const int st = wk.t % ST;
-          mbar_wait(smem_u32(&bar_kv_empty[st]), ((wk.t / ST) & 1) ^ 1);
+          mbar_wait(smem_u32(&bar_k_empty[st]), ((wk.t / ST) & 1) ^ 1);
           mbar_arrive_expect_tx(smem_u32(&bar_k_full[st]), TILE);
           tma_load_5d(sK + st * TILE, &mapK, smem_u32(&bar_k_full[st]), 0, wk.h, wk.c, wk.j * kTileRows, wk.b);
-          // a partially valid last tile goes through the tail fixer (warp 11) before the MMA sees it
+          mbar_wait(smem_u32(&bar_v_empty[st]), ((wk.t / ST) & 1) ^ 1);
+          // a partially valid last tile goes through the tail fix (warp 9) before the PV MMAs see it
           const bool tail = wk.j == wk.tiles - 1 && wk.n % kTileRows != 0;
           const uint32_t vbar = tail ? smem_u32(&bar_v_land[st]) : smem_u32(&bar_v_full[st]);
           mbar_arrive_expect_tx(vbar, TILE);
           tma_load_5d(sV + st * TILE, &mapV, vbar, 0, wk.h, wk.c, wk.j * kTileRows, wk.b);
         }
       }
-    } else if (warp == 9) {
-      // ------------------------------------------------------------------ MMA issuer (one lane)
-      // Everything per MMA is an add on a precomputed descriptor: the first build of this kernel was
-      // bound by the instruction stream of this warp (profiles/r01_s7_full.md).
-      if (lane == 0) {
+    } else {
+      // ------------------------------------------------------------------ MMA issuers
+      // warp 9: S_t = Q_t K_j^T for both query tiles (runs ahead as far as the S buffers allow) and the
+      // V tail fix; warp 10 / 11: O_t += P_t V_j for query tile t = 0 / 1.  Each warp runs its loop
+      // convergently (elect.sync inside every issue) on precomputed descriptors.  One issuing warp costs
+      // ~65 clk per tcgen05.mma (a dependent chain of ~10 SASS instructions), which bound the first two
+      // builds of this kernel (profiles/r01_s7_full.md, r01_s14_item.md); three warps in parallel do not.
+      constexpr uint32_t TILE16 = TILE >> 4;
+      uint32_t st = 0, ph = 0, par = 0, j = 0, tiles = 0, k = 0;
+      int w = blockIdx.x, n = 0;
+      auto seek = [&]() {
+        for (; w < n_items; w += gridDim.x) {
+          const int bc = w / (blocks_per_seq * s.H);
+          if (s.col_valid && __ldg(s.col_valid + bc) == 0) continue;
+          n = clamp_n(s, bc / s.C);
+          tiles = (uint32_t)(n + kTileRows - 1) / kTileRows;
+          return true;
+        }
+        return false;
+      };
+      bool ok = seek();
+      if (warp == 9) {
         constexpr uint32_t idS = make_idesc_bf16(128, 128, false, false);
-        constexpr uint32_t idO = make_idesc_bf16(128, DH, false, true);
-        constexpr uint32_t TILE16 = TILE >> 4;
         const uint64_t dQ = make_smem_desc<ROWB>(sQ, 16, 8 * ROWB);
         const uint64_t dK = make_smem_desc<ROWB>(sK, 16, 8 * ROWB);
-        const uint64_t dV = make_smem_desc<ROWB>(sV, 16, 8 * ROWB);
-        const uint32_t b_k_full = smem_u32(&bar_k_full[0]), b_v_full = smem_u32(&bar_v_full[0]),
-                       b_kv_empty = smem_u32(&bar_kv_empty[0]), b_q_full = smem_u32(&bar_q_full[0]),
-                       b_q_empty = smem_u32(&bar_q_empty[0]), b_s_full = smem_u32(&bar_s_full[0]),
-                       b_s_empty = smem_u32(&bar_s_empty[0]), b_p_full = smem_u32(&bar_p_full[0]),
-                       b_pv_done = smem_u32(&bar_pv_done[0]);
-        // S stream (one tile ahead) and PV stream: ring slot, ring phase, tile parity, item counters
-        uint32_t a_st = 0, a_ph = 0, a_par = 0, a_j = 0, a_tiles = 0, a_k = 0;
-        uint32_t p_st = 0, p_ph = 0, p_par = 0, p_j = 0, p_tiles = 0;
-        int a_w = blockIdx.x, p_w = blockIdx.x;
-        auto seek = [&](int& w, uint32_t& tiles) {
-          for (; w < n_items; w += gridDim.x) {
-            const int bc = w / (blocks_per_seq * s.H);
-            if (s.col_valid && __ldg(s.col_valid + bc) == 0) continue;
-            tiles = (uint32_t)(clamp_n(s, bc / s.C) + kTileRows - 1) / kTileRows;
-            return true;
-          }
-          return false;
-        };
-        bool a_ok = seek(a_w, a_tiles), p_ok = a_ok;
-        p_tiles = a_tiles;
-        p_w = a_w;
-        auto issue_s = [&]() {
-          const uint32_t qb = a_k & 1;
-          if (a_j == 0) mbar_wait(b_q_full + 8 * qb, (a_k >> 1) & 1);
-          mbar_wait(b_k_full + 8 * a_st, a_ph);
-          const uint64_t kd = dK + a_st * TILE16;
+        const uint32_t b_k_full = smem_u32(&bar_k_full[0]), b_k_empty = smem_u32(&bar_k_empty[0]),
+                       b_q_full = smem_u32(&bar_q_full[0]), b_q_empty = smem_u32(&bar_q_empty[0]),
+                       b_s_full = smem_u32(&bar_s_full[0]), b_s_empty = smem_u32(&bar_s_empty[0]);
+        uint32_t tph = 0;  // per-slot phase bits of bar_v_land
+        while (ok) {
+          const uint32_t qb = k & 1;
+          if (j == 0) mbar_wait(b_q_full + 8 * qb, (k >> 1) & 1);
+          mbar_wait(b_k_full + 8 * st, ph);
+          const uint64_t kd = dK + st * TILE16;
 #pragma unroll
           for (int t = 0; t < 2; ++t) {
             const uint64_t qd = dQ + (2 * qb + t) * TILE16;
-            mbar_wait(b_s_empty + 8 * t, a_par ^ 1);
+            mbar_wait(b_s_empty + 8 * t, par ^ 1);
             tc_fence_after();
 #pragma unroll
-            for (int k = 0; k < DH / 16; ++k) mma_ss(tmem + Cfg::S0 + 128 * t, qd + 2 * k, kd + 2 * k, idS, k > 0);
-            tc_commit(b_s_full + 8 * t);
+            for (int kk = 0; kk < DH / 16; ++kk)
+              mma_ss_e(tmem + Cfg::S0 + 128 * t, qd + 2 * kk, kd + 2 * kk, idS, kk > 0);
+            tc_commit_e(b_s_full + 8 * t);
           }
-          a_par ^= 1;
-          if (++a_st == ST) { a_st = 0; a_ph ^= 1; }
-          if (++a_j == a_tiles) {
-            tc_commit(b_q_empty + 8 * qb);
-            a_j = 0;
-            ++a_k;
-            a_w += gridDim.x;
-            a_ok = seek(a_w, a_tiles);
+          tc_commit_e(b_k_empty + 8 * st);
+          if (j == tiles - 1) {
+            tc_commit_e(b_q_empty + 8 * qb);
+            // The last key tile of an item with n % 128 != 0 holds rows >= n_train (test rows).  Their S
+            // columns are masked to -inf by the softmax threads (P = 0), but 0 x (Inf/NaN) would still
+            // poison O, so those V rows are zeroed in shared memory: the producer lands such a tile on
+            // bar_v_land and this warp completes bar_v_full in the TMA's place.
+            const int rem = n - (int)(tiles - 1) * kTileRows;
+            if (rem != kTileRows) {
+              mbar_wait(smem_u32(&bar_v_land[0]) + 8 * st, (tph >> st) & 1);
+              tph ^= 1u << st;
+              zero_tail_rows<ROWB>(sV + st * TILE, rem, lane);
+              if (lane == 0) mbar_arrive(smem_u32(&bar_v_full[0]) + 8 * st);
+            }
           }
-        };
-        auto issue_o = [&]() {
-          mbar_wait(b_v_full + 8 * p_st, p_ph);
-          const uint64_t vd = dV + p_st * TILE16;
-#pragma unroll
-          for (int t = 0; t < 2; ++t) {
-            mbar_wait(b_p_full + 8 * t, p_par);
-            tc_fence_after();
-#pragma unroll
-            for (int kk = 0; kk < kTileRows / 16; ++kk)
-              mma_ts(tmem + Cfg::O0 + DH * t, tmem + Cfg::P0 + 64 * t + 8 * kk, vd + kk * ROWB, idO,
-                     (p_j > 0 || kk > 0) ? 1u : 0u);
-            tc_commit(b_pv_done + 8 * t);
+          par ^= 1;
+          if (++st == ST) { st = 0; ph ^= 1; }
+          if (++j == tiles) {
+            j = 0;
+            ++k;
+            w += gridDim.x;
+            ok = seek();
           }
-          tc_commit(b_kv_empty + 8 * p_st);
-          p_par ^= 1;
-          if (++p_st == ST) { p_st = 0; p_ph ^= 1; }
-          if (++p_j == p_tiles) {
-            p_j = 0;
-            p_w += gridDim.x;
-            p_ok = seek(p_w, p_tiles);
-          }
-        };
-        if (a_ok) issue_s();
-        while (p_ok) {
-          if (a_ok) issue_s();
-          issue_o();
         }
-      }
-      __syncwarp();
-    } else if (warp == 11) {
-      // ------------------------------------------------------------------ V tail fixer
-      // The last key tile of an item with n % 128 != 0 holds rows >= n_train (test rows).  Their S
-      // columns are masked to -inf by the softmax threads (P = 0), but 0 x (Inf/NaN) would still
-      // poison O, so the V rows are zeroed in shared memory.  The producer lands such a tile on
-      // bar_v_land; this warp zeroes the tail and then completes bar_v_full in the TMA's place.
-      uint32_t t = 0, tph = 0;
-      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-        const int bc = w / (blocks_per_seq * s.H);
-        if (s.col_valid && __ldg(s.col_valid + bc) == 0) continue;
-        const int n = clamp_n(s, bc / s.C);
-        const uint32_t tiles = (uint32_t)(n + kTileRows - 1) / kTileRows;
-        t += tiles;
-        const int rem = n - (int)(tiles - 1) * kTileRows;
-        if (rem == kTileRows) continue;
-        const uint32_t st = (t - 1) % ST;
-        mbar_wait(smem_u32(&bar_v_land[st]), (tph >> st) & 1);
-        tph ^= 1u << st;
-        zero_tail_rows<ROWB>(sV + st * TILE, rem, lane);
-        if (lane == 0) mbar_arrive(smem_u32(&bar_v_full[st]));
+      } else if (warp <= 11) {
+        const uint32_t t = warp - 10;
+        constexpr uint32_t idO = make_idesc_bf16(128, DH, false, true);
+        const uint64_t dV = make_smem_desc<ROWB>(sV, 16, 8 * ROWB);
+        const uint32_t b_v_full = smem_u32(&bar_v_full[0]), b_v_empty = smem_u32(&bar_v_empty[0]),
+                       b_p_full = smem_u32(&bar_p_full[t]), b_pv_done = smem_u32(&bar_pv_done[t]);
+        const uint32_t tO = tmem + Cfg::O0 + DH * t, tP = tmem + Cfg::P0 + 64 * t;
+        while (ok) {
+          mbar_wait(b_v_full + 8 * st, ph);
+          const uint64_t vd = dV + st * TILE16;
+          mbar_wait(b_p_full, par);
+          tc_fence_after();
+#pragma unroll
+          for (int kk = 0; kk < kTileRows / 16; ++kk)
+            mma_ts_e(tO, tP + 8 * kk, vd + kk * ROWB, idO, (j > 0 || kk > 0) ? 1u : 0u);
+          tc_commit_e(b_pv_done);
+          tc_commit_e(b_v_empty + 8 * st);
+          par ^= 1;
+          if (++st == ST) { st = 0; ph ^= 1; }
+          if (++j == tiles) {
+            j = 0;
+            w += gridDim.x;
+            ok = seek();
+          }
+        }
       }
     }
   } else {
