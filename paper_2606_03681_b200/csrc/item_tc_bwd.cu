@@ -14,16 +14,18 @@
 // with P = exp2(S * scale*log2e - LSE*log2e) recomputed from the saved LSE.  S/dP accumulate in
 // TMEM (fp32); P and dS go back to TMEM as bf16 and are the A operands of the second-stage MMAs.
 //
-// Warp roles (384 threads, one persistent CTA per SM):
+// Warp roles (512 threads, one persistent CTA per SM; setmaxnreg gives the score warpgroups 168
+// registers and leaves the issuing warps 80):
 //   warp 8   TMA producer (one lane): stationary tiles (double-buffered over items), ring of chunk
 //            pairs (+ the chunk's LSE/D vectors by 1-D bulk copy in MODE_DKV)
-//   warp 9   issuer of the score MMAs (S, dP), two chunks ahead of the accumulation MMAs
-//   warp 10  issuer of the accumulation MMAs (one lane); owns the TMEM allocation
+//   warp 9   issuer of the S MMAs, warp 10 issuer of the dP MMAs (both run ahead of the accumulation
+//            as far as the two TMEM sets allow); warp 10 owns the TMEM allocation
+//   warp 11  issuer of the acc0 MMAs (dQ or dV), warp 12 of the acc1 MMAs (dK, MODE_DKV only)
 //   warpgroups 0/1 = "set" 0/1: each owns one TMEM set (S, dP, dS, P) and takes every other chunk,
 //            one thread per tile row.
-// Every role walks the same item list with its own counters; the per-chunk work of the single-lane
-// roles is a few waits plus the MMA/TMA issues on precomputed descriptors (the first build of this
-// file was bound by the issue rate of its one MMA warp, profiles/r01_tc_launches.md).
+// Every role walks the same item list with its own counters.  An issuing warp needs ~65 clk per
+// tcgen05.mma (a dependent chain of ~10 SASS instructions), which bound the earlier builds of this
+// file (profiles/r01_tc_launches.md, r01_s7_full.md): hence one warp per MMA group.
 #include <cuda.h>
 
 #include <algorithm>
@@ -42,7 +44,8 @@ using namespace itc;
 
 constexpr int MODE_DQ = 0, MODE_DKV = 1;
 constexpr int kChunk = 64;
-constexpr int kBwdThreads = 384;
+constexpr int kBwdThreads = 512;
+__host__ __device__ constexpr int kAccWarps(int mode) { return mode == 0 ? 1 : 2; }
 
 template <int DH>
 struct BwdCfg {
@@ -154,17 +157,17 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&bar_a_full[i]), 1);
-      mbar_init(smem_u32(&bar_a_empty[i]), 1);
-      mbar_init(smem_u32(&bar_s_full[i]), 1);
+      mbar_init(smem_u32(&bar_a_empty[i]), 2);   // S and dP issuers
+      mbar_init(smem_u32(&bar_s_full[i]), 2);    // S and dP issuers
       mbar_init(smem_u32(&bar_s_empty[i]), 4);   // one arrive per warp of the set's warpgroup
       mbar_init(smem_u32(&bar_p_full[i]), 4);
-      mbar_init(smem_u32(&bar_p_empty[i]), 1);
+      mbar_init(smem_u32(&bar_p_empty[i]), kAccWarps(MODE));
     }
     for (int i = 0; i < ST; ++i) {
       mbar_init(smem_u32(&bar_b_full[i]), 1);
-      mbar_init(smem_u32(&bar_b_empty[i]), 1);
+      mbar_init(smem_u32(&bar_b_empty[i]), kAccWarps(MODE));
     }
-    mbar_init(smem_u32(&bar_acc_full), 1);
+    mbar_init(smem_u32(&bar_acc_full), kAccWarps(MODE));
     mbar_init(smem_u32(&bar_acc_free), 8);
     fence_barrier_init();
   }
@@ -173,7 +176,9 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   const int d = s.H * DH;
-
+  // 512 threads start with 128 registers each; the score warpgroups take 168, the issuing warps keep 80
+  if (warp >= 8) {
+  setmaxnreg_dec<80>();
   if (warp == 8) {
     // ------------------------------------------------------------------ producer (one lane)
     if (lane == 0) {
@@ -205,82 +210,85 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         ++k;
       }
     }
-  } else if (warp == 9) {
-    // ------------------------------------------------------------------ score MMAs (S, dP)
-    // Chunk t of the CTA's lifetime uses TMEM set t & 1 and ring stage t % ST.  The whole warp walks
-    // the loop (the tail zeroing needs all lanes); lane 0 issues.
+  } else if (warp == 9 || warp == 10) {
+    // ------------------------------------------------------------------ score MMAs: warp 9 S, warp 10 dP
+    // Chunk t of the CTA's lifetime uses TMEM set t & 1 and ring stage t % ST.  Each warp walks its loop
+    // convergently (elect.sync inside every issue); one issuing warp costs ~65 clk per tcgen05.mma, so
+    // the four MMA groups of a chunk are spread over four warps (profiles/r01_s14_item.md).
     constexpr uint32_t idesc = make_idesc_bf16(128, kChunk, false, false);
-    const uint64_t dA = make_smem_desc<ROWB>(sA, 16, 8 * ROWB);
-    const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
-    uint32_t t = 0, k = 0;
+    const bool is_s = warp == 9;
+    const uint64_t dA = make_smem_desc<ROWB>(sA + (is_s ? 0 : TILE_A), 16, 8 * ROWB);
+    const uint64_t dB = make_smem_desc<ROWB>(sB + (is_s ? 0 : TILE_B), 16, 8 * ROWB);
+    const uint32_t dcol = is_s ? Cfg::S_OFF : Cfg::DP_OFF;
+    const uint32_t b_a_full = smem_u32(&bar_a_full[0]), b_a_empty = smem_u32(&bar_a_empty[0]),
+                   b_b_full = smem_u32(&bar_b_full[0]), b_s_full = smem_u32(&bar_s_full[0]),
+                   b_s_empty = smem_u32(&bar_s_empty[0]);
+    uint32_t t = 0, k = 0, st = 0, ph = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
-      mbar_wait(smem_u32(&bar_a_full[ab]), (k >> 1) & 1);
-      const uint64_t a1 = dA + ((2 * ab) * TILE_A >> 4), a2 = a1 + (TILE_A >> 4);
+      mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
+      const uint64_t a = dA + ((2 * ab) * TILE_A >> 4);
       for (int j = 0; j < it.chunks; ++j, ++t) {
-        const uint32_t st = t % ST, g = t & 1;
-        mbar_wait(smem_u32(&bar_b_full[st]), (t / ST) & 1);
-        if (MODE == MODE_DQ) {
-          const int rem = it.n - j * kChunk;  // keys >= n must not reach dQ through dS K
+        const uint32_t g = t & 1;
+        mbar_wait(b_b_full + 8 * st, ph);
+        if (MODE == MODE_DQ && is_s) {
+          // keys >= n must not reach dQ through dS K: zero the K rows beyond n (dS is forced to 0 there,
+          // but 0 x NaN would still be NaN).  Ordered before the accumulation MMAs of this chunk through
+          // S MMA -> bar_s_full -> score warpgroup -> bar_p_full.
+          const int rem = it.n - j * kChunk;
           if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
-        if (lane == 0) {
-          mbar_wait(smem_u32(&bar_s_empty[g]), ((t >> 1) & 1) ^ 1);
-          tc_fence_after();
-          const uint32_t set = tmem + g * Cfg::SET;
-          const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
+        mbar_wait(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t dst = tmem + g * Cfg::SET + dcol;
+        const uint64_t b = dB + (st * Cfg::STAGE >> 4);
 #pragma unroll
-          for (int kk = 0; kk < DH / 16; ++kk) mma_ss(set + Cfg::S_OFF, a1 + 2 * kk, b1 + 2 * kk, idesc, kk > 0);
-#pragma unroll
-          for (int kk = 0; kk < DH / 16; ++kk) mma_ss(set + Cfg::DP_OFF, a2 + 2 * kk, b2 + 2 * kk, idesc, kk > 0);
-          tc_commit(smem_u32(&bar_s_full[g]));
-          if (j == it.chunks - 1) tc_commit(smem_u32(&bar_a_empty[ab]));
-        }
-        __syncwarp();
+        for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(dst, a + 2 * kk, b + 2 * kk, idesc, kk > 0);
+        tc_commit_e(b_s_full + 8 * g);
+        if (j == it.chunks - 1) tc_commit_e(b_a_empty + 8 * ab);
+        if (++st == ST) { st = 0; ph ^= 1; }
       }
       ++k;
     }
-  } else if (warp == 10) {
-    // ------------------------------------------------------------------ accumulation MMAs (one lane)
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(128, DH, false, true);
-      const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
-      uint32_t t = 0, k = 0;
-      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-        const Item it = decode_item<MODE>(s, w, blocks_per_seq);
-        if (!it.valid) continue;
-        mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
-        for (int j = 0; j < it.chunks; ++j, ++t) {
-          const uint32_t st = t % ST, g = t & 1;
-          mbar_wait(smem_u32(&bar_p_full[g]), (t >> 1) & 1);
-          tc_fence_after();
-          const uint32_t set = tmem + g * Cfg::SET;
-          const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
-          // A = 128 x 64 bf16 in TMEM (8 columns per 16-wide k step); B = 16 chunk rows per k step
-          if (MODE == MODE_DQ) {
+  } else if (warp == 11 || (warp == 12 && MODE == MODE_DKV)) {
+    // ------------------------------------------------------------------ accumulation MMAs
+    // warp 11: acc0 (dQ += dS K, or dV += P^T dO); warp 12 (MODE_DKV): acc1 (dK += dS^T Q)
+    constexpr uint32_t idesc = make_idesc_bf16(128, DH, false, true);
+    const bool first = warp == 11;
+    // A = 128 x 64 bf16 in TMEM (8 columns per 16-wide k step); B = 16 chunk rows per k step
+    const uint32_t acol = (MODE == MODE_DQ || !first) ? Cfg::DS_OFF : Cfg::P_OFF;
+    const uint32_t acc = tmem + (first ? Cfg::ACC0 : Cfg::ACC1);
+    // B operand: dQ <- K chunk (B1); dV <- dO chunk (B2); dK <- Q chunk (B1)
+    const uint64_t dB = make_smem_desc<ROWB>(sB + ((MODE == MODE_DKV && first) ? TILE_B : 0), 16, 8 * ROWB);
+    const uint32_t b_p_full = smem_u32(&bar_p_full[0]), b_p_empty = smem_u32(&bar_p_empty[0]),
+                   b_b_empty = smem_u32(&bar_b_empty[0]);
+    uint32_t t = 0, k = 0, st = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+      if (!it.valid) continue;
+      mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
+      for (int j = 0; j < it.chunks; ++j, ++t) {
+        const uint32_t g = t & 1;
+        mbar_wait(b_p_full + 8 * g, (t >> 1) & 1);
+        tc_fence_after();
+        const uint32_t a = tmem + g * Cfg::SET + acol;
+        const uint64_t b = dB + (st * Cfg::STAGE >> 4);
 #pragma unroll
-            for (int kk = 0; kk < kChunk / 16; ++kk)
-              mma_ts(tmem + Cfg::ACC0, set + Cfg::DS_OFF + 8 * kk, b1 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
-          } else {
-#pragma unroll
-            for (int kk = 0; kk < kChunk / 16; ++kk)
-              mma_ts(tmem + Cfg::ACC0, set + Cfg::P_OFF + 8 * kk, b2 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
-#pragma unroll
-            for (int kk = 0; kk < kChunk / 16; ++kk)
-              mma_ts(tmem + Cfg::ACC1, set + Cfg::DS_OFF + 8 * kk, b1 + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
-          }
-          tc_commit(smem_u32(&bar_p_empty[g]));
-          tc_commit(smem_u32(&bar_b_empty[st]));
-          if (j == it.chunks - 1) tc_commit(smem_u32(&bar_acc_full));
-        }
-        ++k;
+        for (int kk = 0; kk < kChunk / 16; ++kk)
+          mma_ts_e(acc, a + 8 * kk, b + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
+        tc_commit_e(b_p_empty + 8 * g);
+        tc_commit_e(b_b_empty + 8 * st);
+        if (j == it.chunks - 1) tc_commit_e(smem_u32(&bar_acc_full));
+        if (++st == ST) st = 0;
       }
+      ++k;
     }
-    __syncwarp();
-  } else if (warp < 8) {
+  }
+  } else {
     // -------------------------------------------------------------------- score warpgroups (sets)
+    setmaxnreg_inc<168>();
     const int g = warp >> 2;                 // TMEM set / chunk parity of this warpgroup
     const int r = threadIdx.x & 127;         // tile row = TMEM lane
     const uint32_t lane_base = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
