@@ -191,14 +191,14 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         const Item it = decode_item<MODE>(s, w, blocks_per_seq);
         if (!it.valid) continue;
         const uint32_t ab = k & 1, a_full = smem_u32(&bar_a_full[ab]);
-        mbar_wait(smem_u32(&bar_a_empty[ab]), ((k >> 1) & 1) ^ 1);
+        mbar_wait<true>(smem_u32(&bar_a_empty[ab]), ((k >> 1) & 1) ^ 1);
         mbar_arrive_expect_tx(a_full, 2 * TILE_A);
         tma_load_5d(sA + (2 * ab) * TILE_A, &mapA1, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
         tma_load_5d(sA + (2 * ab + 1) * TILE_A, &mapA2, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
         const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
         for (int j = 0; j < it.chunks; ++j, ++t) {
           const uint32_t st = t % ST, b_full = smem_u32(&bar_b_full[st]);
-          mbar_wait(smem_u32(&bar_b_empty[st]), ((t / ST) & 1) ^ 1);
+          mbar_wait<true>(smem_u32(&bar_b_empty[st]), ((t / ST) & 1) ^ 1);
           mbar_arrive_expect_tx(b_full, Cfg::STAGE + (MODE == MODE_DKV ? Cfg::LD_BYTES : 0));
           tma_load_5d(sB + st * Cfg::STAGE, &mapB1, b_full, 0, it.h, it.c, j * kChunk, it.b);
           tma_load_5d(sB + st * Cfg::STAGE + TILE_B, &mapB2, b_full, 0, it.h, it.c, j * kChunk, it.b);
@@ -228,11 +228,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
-      mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
+      mbar_wait<true>(b_a_full + 8 * ab, (k >> 1) & 1);
       const uint64_t a = dA + ((2 * ab) * TILE_A >> 4);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
-        mbar_wait(b_b_full + 8 * st, ph);
+        mbar_wait<true>(b_b_full + 8 * st, ph);
         if (MODE == MODE_DQ && is_s) {
           // keys >= n must not reach dQ through dS K: zero the K rows beyond n (dS is forced to 0 there,
           // but 0 x NaN would still be NaN).  Ordered before the accumulation MMAs of this chunk through
@@ -240,7 +240,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           const int rem = it.n - j * kChunk;
           if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
-        mbar_wait(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
+        mbar_wait<true>(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
         tc_fence_after();
         const uint32_t dst = tmem + g * Cfg::SET + dcol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -268,10 +268,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       if (!it.valid) continue;
-      mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
+      mbar_wait<true>(smem_u32(&bar_acc_free), (k & 1) ^ 1);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
-        mbar_wait(b_p_full + 8 * g, (t >> 1) & 1);
+        mbar_wait<true>(b_p_full + 8 * g, (t >> 1) & 1);
         tc_fence_after();
         const uint32_t a = tmem + g * Cfg::SET + acol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -326,7 +326,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
-        mbar_wait(b_s_full, u & 1);
+        mbar_wait<true>(b_s_full, u & 1);
         tc_fence_after();
         uint32_t sr[64], dr[64];
         tmem_ld32(set + Cfg::S_OFF, sr);
@@ -339,23 +339,24 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         if (lane == 0) mbar_arrive(b_s_empty);
         uint32_t pds[32], pp[32];
         if (MODE == MODE_DQ) {
-          const int rem = it.n - j * kChunk;
 #pragma unroll
           for (int k = 0; k < 64; k += 2) {
             const float p0 = fast_exp2(fmaf(__uint_as_float(sr[k]), c2, -lse2));
             const float p1 = fast_exp2(fmaf(__uint_as_float(sr[k + 1]), c2, -lse2));
-            float d0 = p0 * (__uint_as_float(dr[k]) - Drow);
-            float d1 = p1 * (__uint_as_float(dr[k + 1]) - Drow);
-            if (rem < kChunk) {  // keys >= n_train: dS = 0 exactly, whatever the masked K/V hold
-              d0 = k < rem ? d0 : 0.f;
-              d1 = k + 1 < rem ? d1 : 0.f;
+            pds[k >> 1] = pack_bf16(p0 * (__uint_as_float(dr[k]) - Drow), p1 * (__uint_as_float(dr[k + 1]) - Drow));
+          }
+          const int rem = it.n - j * kChunk;
+          if (rem < kChunk) {  // last chunk only: keys >= n_train get dS = 0 exactly, whatever the masked K/V hold
+#pragma unroll
+            for (int k = 0; k < 32; ++k) {
+              const uint32_t keep = (2 * k < rem ? 0x0000ffffu : 0u) | (2 * k + 1 < rem ? 0xffff0000u : 0u);
+              pds[k] &= keep;
             }
-            pds[k >> 1] = pack_bf16(d0, d1);
           }
         } else {
           const uint32_t st = (tbase + j) % ST;
           // the chunk's LSE/D vectors landed with the chunk (same mbarrier as the score MMAs waited on)
-          mbar_wait(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
+          mbar_wait<true>(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
           const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + st * (2 * kChunk));
           const float4* d4 = l4 + kChunk / 4;
 #pragma unroll
@@ -372,7 +373,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                 pack_bf16(p2 * (__uint_as_float(dr[k + 2]) - Dv.z), p3 * (__uint_as_float(dr[k + 3]) - Dv.w));
           }
         }
-        mbar_wait(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
+        mbar_wait<true>(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
         tmem_st32(set + Cfg::DS_OFF, pds);
         if (MODE == MODE_DKV) tmem_st32(set + Cfg::P_OFF, pp);
         tmem_wait_st();
@@ -381,7 +382,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         if (lane == 0) mbar_arrive(b_p_full);
       }
       // ---- epilogue ---------------------------------------------------------------------------------
-      mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
+      mbar_wait<true>(smem_u32(&bar_acc_full), kitem & 1);
       tc_fence_after();
       if (MODE == MODE_DQ) {
         constexpr int HALF = DH / 2;  // each warpgroup stores half of the dQ columns of its row
