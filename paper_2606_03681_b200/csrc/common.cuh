@@ -66,4 +66,75 @@ __device__ __forceinline__ float fast_exp2(float x) {
   return y;
 }
 
+
+// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2, two fp32 lanes per issue slot) ---------
+__device__ __forceinline__ uint64_t f2pack(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2unpack(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
+// 2^x for two values on the FMA pipe instead of the MUFU (16 ex2/clk/SM is the ceiling of the item
+// kernels at dh <= 64): x is clamped to >= -126, split as n + f with n = round(x)
+// (magic-number add) and f in [-0.5, 0.5]; 2^f by a cubic (max relative error 2.0e-4, an eighth of
+// the bf16 rounding step the result is rounded to); 2^n by adding n to the exponent field.
+// x = -inf (masked score) gives 2^-126 instead of 0: callers multiply it by zeroed operands or mask it.
+__device__ __forceinline__ void exp2_poly2(uint64_t x, float& e0, float& e1) {
+  float a, b;
+  f2unpack(x, a, b);
+  const uint64_t v = f2pack(fmaxf(a, -126.f), fmaxf(b, -126.f));
+  const uint64_t magic = f2pack(12582912.f, 12582912.f);  // 1.5 * 2^23
+  const uint64_t t = add2(v, magic);
+  const uint64_t f = sub2(v, sub2(t, magic));
+  uint64_t p = fma2(f2pack(0.053027521818876266f, 0.053027521818876266f), f,
+                    f2pack(0.24221394956111908f, 0.24221394956111908f));
+  p = fma2(p, f, f2pack(0.6935725808143616f, 0.6935725808143616f));
+  p = fma2(p, f, f2pack(0.9999590516090393f, 0.9999590516090393f));
+  float pl, ph, tl, th;
+  f2unpack(p, pl, ph);
+  f2unpack(t, tl, th);
+  e0 = __int_as_float(__float_as_int(pl) + (__float_as_int(tl) << 23));
+  e1 = __int_as_float(__float_as_int(ph) + (__float_as_int(th) << 23));
+}
+// 2^x for a pair: the polynomial when POLY, else two MUFU ex2
+// (`poly` is a compile-time constant after unrolling the caller's loop)
+__device__ __forceinline__ void exp2_pair(bool poly, uint64_t x, float& e0, float& e1) {
+  if (poly) {
+    exp2_poly2(x, e0, e1);
+  } else {
+    float a, b;
+    f2unpack(x, a, b);
+    e0 = fast_exp2(a);
+    e1 = fast_exp2(b);
+  }
+}
+// which pairs of an unrolled loop take the polynomial: kPolyOf8 of every 8 consecutive pairs, spread out
+template <int POLY_OF_8>
+__host__ __device__ constexpr bool pair_is_poly(int k) {
+  return ((k % 8) * POLY_OF_8) / 8 != (((k % 8) + 1) * POLY_OF_8) / 8;
+}
+
 }  // namespace tabattn

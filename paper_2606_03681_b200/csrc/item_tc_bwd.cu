@@ -60,6 +60,8 @@ struct BwdCfg {
   static constexpr int SET = 192, S_OFF = 0, DP_OFF = 64, DS_OFF = 128, P_OFF = 160;
   static constexpr int ACC0 = 384, ACC1 = 384 + DH, COLS = 512;
   static_assert(ACC1 + DH <= COLS, "TMEM budget");
+  // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2, common.cuh) instead of the MUFU
+  static constexpr int POLY_OF_8 = DH >= 64 ? 0 : 2;
 };
 
 // One work item = (table b, column c, head h, 128-row block blk) of the stationary axis.
@@ -90,7 +92,7 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
                : "memory");
 }
 
-// ---- prep: D[b,c,h,r] = sum_k dO O, lse2 = LSE * log2(e); rows r in [R, Rp) get D = 0, lse2 = +inf ------
+// ---- prep: D[b,c,h,r] = sum_k dO O, nlse2 = -LSE * log2(e); rows r in [R, Rp) get D = 0, nlse2 = -inf ----
 // One CTA = 32 rows of one (b, c); the two outputs are [B*C*H][Rp] f32 (Rp = R rounded up to 64).
 __global__ void __launch_bounds__(256) item_bwd_prep_kernel(Shape s, const __nv_bfloat16* __restrict__ O,
                                                             const __nv_bfloat16* __restrict__ dO,
@@ -128,7 +130,7 @@ __global__ void __launch_bounds__(256) item_bwd_prep_kernel(Shape s, const __nv_
     if (r >= Rp) continue;
     const size_t seq = ((size_t)bc * s.H + h);
     const bool in = r < s.R;
-    lse2_ws[seq * Rp + r] = in ? __ldg(LSE + seq * s.R + r) * kLog2e : INFINITY;
+    lse2_ws[seq * Rp + r] = in ? -__ldg(LSE + seq * s.R + r) * kLog2e : -INFINITY;
     D_ws[seq * Rp + r] = in ? sD[rr][h] : 0.f;
   }
 }
@@ -317,12 +319,13 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         }
         continue;
       }
-      // per-row constants of the dQ pass (rows >= R: lse2 = +inf -> P = 0)
-      float lse2 = INFINITY, Drow = 0.f;
+      // per-row constants of the dQ pass (rows >= R: nlse2 = -inf -> P = 0)
+      float nlse2 = -INFINITY, Drow = 0.f;
       if (MODE == MODE_DQ && row < Rp) {
-        lse2 = __ldg(lse2_ws + seq + row);
+        nlse2 = __ldg(lse2_ws + seq + row);
         Drow = __ldg(D_ws + seq + row);
       }
+      const uint64_t cc = f2pack(c2, c2), nl = f2pack(nlse2, nlse2), dd = f2pack(Drow, Drow);
       const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
@@ -339,11 +342,15 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         if (lane == 0) mbar_arrive(b_s_empty);
         uint32_t pds[32], pp[32];
         if (MODE == MODE_DQ) {
+          // P = 2^(S*c2 - lse2), dS = P o (dP - D) on packed fp32 pairs
 #pragma unroll
-          for (int k = 0; k < 64; k += 2) {
-            const float p0 = fast_exp2(fmaf(__uint_as_float(sr[k]), c2, -lse2));
-            const float p1 = fast_exp2(fmaf(__uint_as_float(sr[k + 1]), c2, -lse2));
-            pds[k >> 1] = pack_bf16(p0 * (__uint_as_float(dr[k]) - Drow), p1 * (__uint_as_float(dr[k + 1]) - Drow));
+          for (int k = 0; k < 32; ++k) {
+            const uint64_t x = fma2(f2pack(__uint_as_float(sr[2 * k]), __uint_as_float(sr[2 * k + 1])), cc, nl);
+            float p0, p1, d0, d1;
+            exp2_pair(pair_is_poly<Cfg::POLY_OF_8>(k), x, p0, p1);
+            const uint64_t dpd = sub2(f2pack(__uint_as_float(dr[2 * k]), __uint_as_float(dr[2 * k + 1])), dd);
+            f2unpack(mul2(f2pack(p0, p1), dpd), d0, d1);
+            pds[k] = pack_bf16(d0, d1);
           }
           const int rem = it.n - j * kChunk;
           if (rem < kChunk) {  // last chunk only: keys >= n_train get dS = 0 exactly, whatever the masked K/V hold
@@ -357,20 +364,24 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           const uint32_t st = (tbase + j) % ST;
           // the chunk's LSE/D vectors landed with the chunk (same mbarrier as the score MMAs waited on)
           mbar_wait<true>(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
-          const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + st * (2 * kChunk));
-          const float4* d4 = l4 + kChunk / 4;
+          const ulonglong2* l4 = reinterpret_cast<const ulonglong2*>(sLD_ptr + st * (2 * kChunk));
+          const ulonglong2* d4 = l4 + kChunk / 4;
 #pragma unroll
           for (int k = 0; k < 64; k += 4) {
-            const float4 L = l4[k >> 2], Dv = d4[k >> 2];
-            const float p0 = fast_exp2(fmaf(__uint_as_float(sr[k]), c2, -L.x));
-            const float p1 = fast_exp2(fmaf(__uint_as_float(sr[k + 1]), c2, -L.y));
-            const float p2 = fast_exp2(fmaf(__uint_as_float(sr[k + 2]), c2, -L.z));
-            const float p3 = fast_exp2(fmaf(__uint_as_float(sr[k + 3]), c2, -L.w));
+            const ulonglong2 L = l4[k >> 2], Dv = d4[k >> 2];  // (nlse2, D) of query columns k .. k+3
+            float p0, p1, p2, p3, d0, d1, d2, d3;
+            const uint64_t xa = fma2(f2pack(__uint_as_float(sr[k]), __uint_as_float(sr[k + 1])), cc, L.x);
+            const uint64_t xb = fma2(f2pack(__uint_as_float(sr[k + 2]), __uint_as_float(sr[k + 3])), cc, L.y);
+            exp2_pair(pair_is_poly<Cfg::POLY_OF_8>(k >> 1), xa, p0, p1);
+            exp2_pair(pair_is_poly<Cfg::POLY_OF_8>((k >> 1) + 1), xb, p2, p3);
             pp[k >> 1] = pack_bf16(p0, p1);
             pp[(k >> 1) + 1] = pack_bf16(p2, p3);
-            pds[k >> 1] = pack_bf16(p0 * (__uint_as_float(dr[k]) - Dv.x), p1 * (__uint_as_float(dr[k + 1]) - Dv.y));
-            pds[(k >> 1) + 1] =
-                pack_bf16(p2 * (__uint_as_float(dr[k + 2]) - Dv.z), p3 * (__uint_as_float(dr[k + 3]) - Dv.w));
+            const uint64_t da = sub2(f2pack(__uint_as_float(dr[k]), __uint_as_float(dr[k + 1])), Dv.x);
+            const uint64_t db = sub2(f2pack(__uint_as_float(dr[k + 2]), __uint_as_float(dr[k + 3])), Dv.y);
+            f2unpack(mul2(f2pack(p0, p1), da), d0, d1);
+            f2unpack(mul2(f2pack(p2, p3), db), d2, d3);
+            pds[k >> 1] = pack_bf16(d0, d1);
+            pds[(k >> 1) + 1] = pack_bf16(d2, d3);
           }
         }
         mbar_wait<true>(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done

@@ -37,6 +37,9 @@ struct FwdCfg {
   // TMEM columns
   static constexpr int S0 = 0, P0 = 256, O0 = 384, COLS = 512;
   static_assert(O0 + 2 * DH <= COLS, "TMEM budget");
+  // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2) instead of the MUFU: measured
+  // on B200 (profiles/r01_s14_item.md) +8 % at dh = 32, -1.5 % (2 of 8) to -16 % (5 of 8) at dh = 64
+  static constexpr int POLY_OF_8 = DH >= 64 ? 0 : 2;
 };
 
 constexpr int kFwdThreads = 384;
@@ -284,19 +287,24 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           tmem_st_cols<DH>(tO, o);
           tmem_wait_st();
         }
-        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        // P = 2^(S*c2 - m) on packed pairs; Cfg::POLY_OF_8 of every 8 pairs take the FMA-pipe polynomial, the
+        // rest the MUFU, so that the two pipes finish together
+        const uint64_t cc = f2pack(c2, c2), nm = f2pack(-m, -m);
+        uint64_t la = 0, lb = 0;  // two packed partial row sums (+0.f, +0.f)
         uint32_t p[64];
 #pragma unroll
-        for (int k = 0; k < 64; k += 2) {
-          const float e0 = fast_exp2(fmaf(sf[2 * k], c2, -m));
-          const float e1 = fast_exp2(fmaf(sf[2 * k + 1], c2, -m));
-          const float e2 = fast_exp2(fmaf(sf[2 * k + 2], c2, -m));
-          const float e3 = fast_exp2(fmaf(sf[2 * k + 3], c2, -m));
-          l0 += e0; l1 += e1; l2 += e2; l3 += e3;
+        for (int k = 0; k < 64; ++k) {
+          const uint64_t x = fma2(f2pack(sf[2 * k], sf[2 * k + 1]), cc, nm);
+          float e0, e1;
+          exp2_pair(pair_is_poly<Cfg::POLY_OF_8>(k), x, e0, e1);
+          if (k & 1) lb = add2(lb, f2pack(e0, e1)); else la = add2(la, f2pack(e0, e1));
           p[k] = pack_bf16(e0, e1);
-          p[k + 1] = pack_bf16(e2, e3);
         }
-        l += (l0 + l1) + (l2 + l3);
+        {
+          float s0, s1;
+          f2unpack(add2(la, lb), s0, s1);
+          l += s0 + s1;
+        }
         if (g > 0) mbar_wait(b_pv_done, (g - 1) & 1);  // previous PV has finished reading the P buffer
         tmem_st32(tP, p);
         tmem_st32(tP + 32, p + 32);
