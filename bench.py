@@ -345,12 +345,12 @@ def run_ours(args):
         roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": None, "kernel": "tabattn_" + dom, "peak_source": peaks["source"],
                 "algorithmic_bytes_per_launch": nbytes}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # ncu --set full dram bytes per launch
+    traffic_file = os.path.join(ROOT, "profiles", "r01_traffic.csv")   # ncu --set full DRAM bytes per call
     if os.path.exists(traffic_file):
-        try:
-            roof["traffic"] = json.load(open(traffic_file)).get(cfg.name, {}).get(dom)
-        except Exception:
-            pass
+        for row in open(traffic_file).read().splitlines()[1:]:
+            f = row.split(",")
+            if len(f) == 3 and f[0] == cfg.name and f[1] == dom:
+                roof["traffic"] = int(f[2])
     calls = {}
     for n in names:
         ms = call_ms[n]
