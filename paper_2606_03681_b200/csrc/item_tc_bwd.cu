@@ -154,7 +154,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_p_empty[2], bar_acc_full, bar_acc_free;
   __shared__ uint32_t tmem_slot;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // provably warp-uniform
   if (warp == 10) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
