@@ -230,11 +230,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
-      mbar_wait<true>(b_a_full + 8 * ab, (k >> 1) & 1);
+      mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
       const uint64_t a = dA + ((2 * ab) * TILE_A >> 4);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
-        mbar_wait<true>(b_b_full + 8 * st, ph);
+        mbar_wait(b_b_full + 8 * st, ph);
         if (MODE == MODE_DQ && is_s) {
           // keys >= n must not reach dQ through dS K: zero the K rows beyond n (dS is forced to 0 there,
           // but 0 x NaN would still be NaN).  Ordered before the accumulation MMAs of this chunk through
@@ -242,7 +242,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           const int rem = it.n - j * kChunk;
           if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
-        mbar_wait<true>(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
+        mbar_wait(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
         tc_fence_after();
         const uint32_t dst = tmem + g * Cfg::SET + dcol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -270,10 +270,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       const Item it = decode_item<MODE>(s, w, blocks_per_seq);
       if (!it.valid) continue;
-      mbar_wait<true>(smem_u32(&bar_acc_free), (k & 1) ^ 1);
+      mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
-        mbar_wait<true>(b_p_full + 8 * g, (t >> 1) & 1);
+        mbar_wait(b_p_full + 8 * g, (t >> 1) & 1);
         tc_fence_after();
         const uint32_t a = tmem + g * Cfg::SET + acol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -329,7 +329,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
-        mbar_wait<true>(b_s_full, u & 1);
+        mbar_wait(b_s_full, u & 1);
         tc_fence_after();
         uint32_t sr[64], dr[64];
         tmem_ld32(set + Cfg::S_OFF, sr);
@@ -363,7 +363,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         } else {
           const uint32_t st = (tbase + j) % ST;
           // the chunk's LSE/D vectors landed with the chunk (same mbarrier as the score MMAs waited on)
-          mbar_wait<true>(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
+          mbar_wait(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
           const ulonglong2* l4 = reinterpret_cast<const ulonglong2*>(sLD_ptr + st * (2 * kChunk));
           const ulonglong2* d4 = l4 + kChunk / 4;
 #pragma unroll
@@ -384,7 +384,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
             pds[(k >> 1) + 1] = pack_bf16(d2, d3);
           }
         }
-        mbar_wait<true>(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
+        mbar_wait(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
         tmem_st32(set + Cfg::DS_OFF, pds);
         if (MODE == MODE_DKV) tmem_st32(set + Cfg::P_OFF, pp);
         tmem_wait_st();
@@ -393,7 +393,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         if (lane == 0) mbar_arrive(b_p_full);
       }
       // ---- epilogue ---------------------------------------------------------------------------------
-      mbar_wait<true>(smem_u32(&bar_acc_full), kitem & 1);
+      mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
       tc_fence_after();
       if (MODE == MODE_DQ) {
         constexpr int HALF = DH / 2;  // each warpgroup stores half of the dQ columns of its row
