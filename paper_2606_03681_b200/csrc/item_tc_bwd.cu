@@ -14,18 +14,20 @@
 // with P = exp2(S * scale*log2e - LSE*log2e) recomputed from the saved LSE.  S/dP accumulate in
 // TMEM (fp32); P and dS go back to TMEM as bf16 and are the A operands of the second-stage MMAs.
 //
-// Warp roles (512 threads, one persistent CTA per SM; setmaxnreg gives the score warpgroups 168
-// registers and leaves the issuing warps 80):
-//   warp 8   TMA producer (one lane): stationary tiles (double-buffered over items), ring of chunk
-//            pairs (+ the chunk's LSE/D vectors by 1-D bulk copy in MODE_DKV)
-//   warp 9   issuer of the S MMAs, warp 10 issuer of the dP MMAs (both run ahead of the accumulation
-//            as far as the two TMEM sets allow); warp 10 owns the TMEM allocation
-//   warp 11  issuer of the acc0 MMAs (dQ or dV), warp 12 of the acc1 MMAs (dK, MODE_DKV only)
-//   warpgroups 0/1 = "set" 0/1: each owns one TMEM set (S, dP, dS, P) and takes every other chunk,
-//            one thread per tile row.
-// Every role walks the same item list with its own counters.  An issuing warp needs ~65 clk per
-// tcgen05.mma (a dependent chain of ~10 SASS instructions), which bound the earlier builds of this
-// file (profiles/r01_tc_launches.md, r01_s7_full.md): hence one warp per MMA group.
+// Warp roles (640 threads, one persistent CTA per SM; setmaxnreg gives the score warpgroups 104
+// registers and leaves the issuing warps 64):
+//   warps 0-15  four score warpgroups: wg & 1 = TMEM set (S, dP, dS, P) = chunk parity, wg >> 1 = which 32
+//               of the chunk's 64 columns; one thread per (tile row, 32 columns).  Four score warps per
+//               SM sub-partition instead of two: base bwd 1.92 -> 1.79 ms, ragged 8.26 -> 7.77 ms
+//   warp 16     TMA producer (one lane): stationary tiles (double-buffered over items), ring of chunk
+//               pairs (+ the chunk's LSE/D vectors by 1-D bulk copy in MODE_DKV)
+//   warp 17     issuer of the score MMAs (S, dP), runs ahead of the accumulation as far as the two TMEM
+//               sets allow; owns the TMEM allocation
+//   warp 18     issuer of the acc0 MMAs (dQ or dV), warp 19 of the acc1 MMAs (dK, MODE_DKV only)
+// Every role walks the same item list with its own counters.  The issuing warps run convergently with a
+// provably warp-uniform warp index, so ptxas keeps descriptors in uniform registers (~3 SASS instructions
+// per tcgen05.mma; the earlier builds needed ~10-20 and were bound by the issue chain,
+// profiles/r01_tc_launches.md, r01_s7_full.md, r01_s14_item.md).
 #include <cuda.h>
 
 #include <algorithm>
@@ -44,7 +46,8 @@ using namespace itc;
 
 constexpr int MODE_DQ = 0, MODE_DKV = 1;
 constexpr int kChunk = 64;
-constexpr int kBwdThreads = 512;
+constexpr int kScoreWarps = 16;                       // four score warpgroups
+constexpr int kBwdThreads = (kScoreWarps + 4) * 32;   // + producer, score issuer, two accumulation issuers
 __host__ __device__ constexpr int kAccWarps(int mode) { return mode == 0 ? 1 : 2; }
 
 template <int DH>
@@ -155,14 +158,14 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   __shared__ uint32_t tmem_slot;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // provably warp-uniform
-  if (warp == 10) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
+  if (warp == kScoreWarps + 1) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&bar_a_full[i]), 1);
-      mbar_init(smem_u32(&bar_a_empty[i]), 2);   // S and dP issuers
-      mbar_init(smem_u32(&bar_s_full[i]), 2);    // S and dP issuers
-      mbar_init(smem_u32(&bar_s_empty[i]), 4);   // one arrive per warp of the set's warpgroup
-      mbar_init(smem_u32(&bar_p_full[i]), 4);
+      mbar_init(smem_u32(&bar_a_empty[i]), 1);
+      mbar_init(smem_u32(&bar_s_full[i]), 1);
+      mbar_init(smem_u32(&bar_s_empty[i]), 8);   // one arrive per warp of the set's two warpgroups
+      mbar_init(smem_u32(&bar_p_full[i]), 8);
       mbar_init(smem_u32(&bar_p_empty[i]), kAccWarps(MODE));
     }
     for (int i = 0; i < ST; ++i) {
@@ -170,7 +173,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       mbar_init(smem_u32(&bar_b_empty[i]), kAccWarps(MODE));
     }
     mbar_init(smem_u32(&bar_acc_full), kAccWarps(MODE));
-    mbar_init(smem_u32(&bar_acc_free), 8);
+    mbar_init(smem_u32(&bar_acc_free), (MODE == MODE_DQ && DH < 32) ? 8 : 16);   // warps that read the accumulators
     fence_barrier_init();
   }
   tc_fence_before();
@@ -178,10 +181,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   const int d = s.H * DH;
-  // 512 threads start with 128 registers each; the score warpgroups take 168, the issuing warps keep 80
-  if (warp >= 8) {
-  setmaxnreg_dec<80>();
-  if (warp == 8) {
+  // 640 threads start with 96 registers each; the score warpgroups take 104, the issuing warps keep 64
+  // (setmaxnreg can only redistribute the 640 x 96 registers the CTA was launched with)
+  if (warp >= kScoreWarps) {
+  setmaxnreg_dec<64>();
+  if (warp == kScoreWarps) {
     // ------------------------------------------------------------------ producer (one lane)
     if (lane == 0) {
       tma_prefetch_desc(&mapA1);
@@ -212,16 +216,14 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         ++k;
       }
     }
-  } else if (warp == 9 || warp == 10) {
-    // ------------------------------------------------------------------ score MMAs: warp 9 S, warp 10 dP
-    // Chunk t of the CTA's lifetime uses TMEM set t & 1 and ring stage t % ST.  Each warp walks its loop
-    // convergently (elect.sync inside every issue); one issuing warp costs ~65 clk per tcgen05.mma, so
-    // the four MMA groups of a chunk are spread over four warps (profiles/r01_s14_item.md).
+  } else if (warp == kScoreWarps + 1) {
+    // ------------------------------------------------------------------ score MMAs (S, dP)
+    // Chunk t of the CTA's lifetime uses TMEM set t & 1 and ring stage t % ST.  The warp walks its loop
+    // convergently (elect.sync inside every issue; `warp` is provably uniform, so ptxas keeps the
+    // descriptors in uniform registers: ~3 SASS instructions per tcgen05.mma, profiles/r01_s14_item.md).
     constexpr uint32_t idesc = make_idesc_bf16(128, kChunk, false, false);
-    const bool is_s = warp == 9;
-    const uint64_t dA = make_smem_desc<ROWB>(sA + (is_s ? 0 : TILE_A), 16, 8 * ROWB);
-    const uint64_t dB = make_smem_desc<ROWB>(sB + (is_s ? 0 : TILE_B), 16, 8 * ROWB);
-    const uint32_t dcol = is_s ? Cfg::S_OFF : Cfg::DP_OFF;
+    const uint64_t dA = make_smem_desc<ROWB>(sA, 16, 8 * ROWB);
+    const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
     const uint32_t b_a_full = smem_u32(&bar_a_full[0]), b_a_empty = smem_u32(&bar_a_empty[0]),
                    b_b_full = smem_u32(&bar_b_full[0]), b_s_full = smem_u32(&bar_s_full[0]),
                    b_s_empty = smem_u32(&bar_s_empty[0]);
@@ -231,34 +233,36 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
       mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
-      const uint64_t a = dA + ((2 * ab) * TILE_A >> 4);
+      const uint64_t a1 = dA + ((2 * ab) * TILE_A >> 4), a2 = a1 + (TILE_A >> 4);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
         mbar_wait(b_b_full + 8 * st, ph);
-        if (MODE == MODE_DQ && is_s) {
+        if (MODE == MODE_DQ) {
           // keys >= n must not reach dQ through dS K: zero the K rows beyond n (dS is forced to 0 there,
           // but 0 x NaN would still be NaN).  Ordered before the accumulation MMAs of this chunk through
-          // S MMA -> bar_s_full -> score warpgroup -> bar_p_full.
+          // S MMA -> bar_s_full -> score warpgroups -> bar_p_full.
           const int rem = it.n - j * kChunk;
           if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
         mbar_wait(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
         tc_fence_after();
-        const uint32_t dst = tmem + g * Cfg::SET + dcol;
-        const uint64_t b = dB + (st * Cfg::STAGE >> 4);
+        const uint32_t set = tmem + g * Cfg::SET;
+        const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
 #pragma unroll
-        for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(dst, a + 2 * kk, b + 2 * kk, idesc, kk > 0);
+        for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(set + Cfg::S_OFF, a1 + 2 * kk, b1 + 2 * kk, idesc, kk > 0);
+#pragma unroll
+        for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(set + Cfg::DP_OFF, a2 + 2 * kk, b2 + 2 * kk, idesc, kk > 0);
         tc_commit_e(b_s_full + 8 * g);
         if (j == it.chunks - 1) tc_commit_e(b_a_empty + 8 * ab);
         if (++st == ST) { st = 0; ph ^= 1; }
       }
       ++k;
     }
-  } else if (warp == 11 || (warp == 12 && MODE == MODE_DKV)) {
+  } else if (warp == kScoreWarps + 2 || (warp == kScoreWarps + 3 && MODE == MODE_DKV)) {
     // ------------------------------------------------------------------ accumulation MMAs
-    // warp 11: acc0 (dQ += dS K, or dV += P^T dO); warp 12 (MODE_DKV): acc1 (dK += dS^T Q)
+    // first warp: acc0 (dQ += dS K, or dV += P^T dO); second warp (MODE_DKV): acc1 (dK += dS^T Q)
     constexpr uint32_t idesc = make_idesc_bf16(128, DH, false, true);
-    const bool first = warp == 11;
+    const bool first = warp == kScoreWarps + 2;
     // A = 128 x 64 bf16 in TMEM (8 columns per 16-wide k step); B = 16 chunk rows per k step
     const uint32_t acol = (MODE == MODE_DQ || !first) ? Cfg::DS_OFF : Cfg::P_OFF;
     const uint32_t acc = tmem + (first ? Cfg::ACC0 : Cfg::ACC1);
@@ -289,9 +293,12 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     }
   }
   } else {
-    // -------------------------------------------------------------------- score warpgroups (sets)
-    setmaxnreg_inc<168>();
-    const int g = warp >> 2;                 // TMEM set / chunk parity of this warpgroup
+    // -------------------------------------------------------------------- score warpgroups
+    // Four warpgroups: wg = warp >> 2; set g = wg & 1 (TMEM set / chunk parity), column half c = wg >> 1:
+    // the two warpgroups of a set split the chunk's 64 columns, one thread per (tile row, 32 columns).
+    // Four instead of two score warps per SM sub-partition hide each other's MUFU / FMA latencies.
+    setmaxnreg_inc<104>();
+    const int g = (warp >> 2) & 1, c = warp >> 3;
     const int r = threadIdx.x & 127;         // tile row = TMEM lane
     const uint32_t lane_base = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
     const uint32_t set = lane_base + g * Cfg::SET;
@@ -307,7 +314,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
       if (!it.valid) {
         // invalid column, or (MODE_DKV) a key block entirely beyond the train rows: zeros
-        if (row < s.R) {
+        if (row < s.R && c == 0) {
           if (MODE == MODE_DQ) {
 #pragma unroll
             for (int k = 0; k < DH / 16; ++k) stg_v4(out0 + cell + g * (DH / 2) + 8 * k, make_uint4(0, 0, 0, 0));
@@ -331,20 +338,18 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
         mbar_wait(b_s_full, u & 1);
         tc_fence_after();
-        uint32_t sr[64], dr[64];
-        tmem_ld32(set + Cfg::S_OFF, sr);
-        tmem_ld32(set + Cfg::S_OFF + 32, sr + 32);
-        tmem_ld32(set + Cfg::DP_OFF, dr);
-        tmem_ld32(set + Cfg::DP_OFF + 32, dr + 32);
+        uint32_t sr[32], dr[32];
+        tmem_ld32(set + Cfg::S_OFF + 32 * c, sr);
+        tmem_ld32(set + Cfg::DP_OFF + 32 * c, dr);
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(b_s_empty);
-        uint32_t pds[32], pp[32];
+        uint32_t pds[16], pp[16];
         if (MODE == MODE_DQ) {
           // P = 2^(S*c2 - lse2), dS = P o (dP - D) on packed fp32 pairs
 #pragma unroll
-          for (int k = 0; k < 32; ++k) {
+          for (int k = 0; k < 16; ++k) {
             const uint64_t x = fma2(f2pack(__uint_as_float(sr[2 * k]), __uint_as_float(sr[2 * k + 1])), cc, nl);
             float p0, p1, d0, d1;
             exp2_pair(pair_is_poly<Cfg::POLY_OF_8>(k), x, p0, p1);
@@ -352,10 +357,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
             f2unpack(mul2(f2pack(p0, p1), dpd), d0, d1);
             pds[k] = pack_bf16(d0, d1);
           }
-          const int rem = it.n - j * kChunk;
-          if (rem < kChunk) {  // last chunk only: keys >= n_train get dS = 0 exactly, whatever the masked K/V hold
+          const int rem = it.n - j * kChunk - 32 * c;
+          if (rem < 32) {  // last chunk only: keys >= n_train get dS = 0 exactly, whatever the masked K/V hold
 #pragma unroll
-            for (int k = 0; k < 32; ++k) {
+            for (int k = 0; k < 16; ++k) {
               const uint32_t keep = (2 * k < rem ? 0x0000ffffu : 0u) | (2 * k + 1 < rem ? 0xffff0000u : 0u);
               pds[k] &= keep;
             }
@@ -364,11 +369,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           const uint32_t st = (tbase + j) % ST;
           // the chunk's LSE/D vectors landed with the chunk (same mbarrier as the score MMAs waited on)
           mbar_wait(smem_u32(&bar_b_full[st]), ((tbase + j) / ST) & 1);
-          const ulonglong2* l4 = reinterpret_cast<const ulonglong2*>(sLD_ptr + st * (2 * kChunk));
+          const ulonglong2* l4 = reinterpret_cast<const ulonglong2*>(sLD_ptr + st * (2 * kChunk)) + 8 * c;
           const ulonglong2* d4 = l4 + kChunk / 4;
 #pragma unroll
-          for (int k = 0; k < 64; k += 4) {
-            const ulonglong2 L = l4[k >> 2], Dv = d4[k >> 2];  // (nlse2, D) of query columns k .. k+3
+          for (int k = 0; k < 32; k += 4) {
+            const ulonglong2 L = l4[k >> 2], Dv = d4[k >> 2];  // (nlse2, D) of query columns 32c + k .. k+3
             float p0, p1, p2, p3, d0, d1, d2, d3;
             const uint64_t xa = fma2(f2pack(__uint_as_float(sr[k]), __uint_as_float(sr[k + 1])), cc, L.x);
             const uint64_t xb = fma2(f2pack(__uint_as_float(sr[k + 2]), __uint_as_float(sr[k + 3])), cc, L.y);
@@ -385,43 +390,51 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           }
         }
         mbar_wait(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
-        tmem_st32(set + Cfg::DS_OFF, pds);
-        if (MODE == MODE_DKV) tmem_st32(set + Cfg::P_OFF, pp);
+        tmem_st16(set + Cfg::DS_OFF + 16 * c, pds);
+        if (MODE == MODE_DKV) tmem_st16(set + Cfg::P_OFF + 16 * c, pp);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(b_p_full);
       }
       // ---- epilogue ---------------------------------------------------------------------------------
-      mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
-      tc_fence_after();
       if (MODE == MODE_DQ) {
-        constexpr int HALF = DH / 2;  // each warpgroup stores half of the dQ columns of its row
-        uint32_t acc[HALF];
-        tmem_ld_cols<HALF>(lane_base + Cfg::ACC0 + g * HALF, acc);
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
-        if (row < s.R) {
+        // the dQ columns of a row are split over the four warpgroups (two at dh = 16: 16-byte stores)
+        constexpr int EPW = DH >= 32 ? 4 : 2, PART = DH / EPW;
+        const int q = g + 2 * c;
+        if (q < EPW) {
+          mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
+          tc_fence_after();
+          uint32_t acc[PART];
+          tmem_ld_cols<PART>(lane_base + Cfg::ACC0 + q * PART, acc);
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
+          if (row < s.R) {
 #pragma unroll
-          for (int k = 0; k < HALF / 8; ++k) {
-            float f[8];
+            for (int k = 0; k < PART / 8; ++k) {
+              float f[8];
 #pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(acc[8 * k + e]) * s.scale;
-            stg_v4(out0 + cell + g * HALF + 8 * k, pack8(f));
+              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(acc[8 * k + e]) * s.scale;
+              stg_v4(out0 + cell + q * PART + 8 * k, pack8(f));
+            }
           }
         }
       } else {
-        uint32_t acc[DH];  // warpgroup 0: dV = acc0; warpgroup 1: dK = scale * acc1
-        tmem_ld_cols<DH>(lane_base + (g == 0 ? Cfg::ACC0 : Cfg::ACC1), acc);
+        // set 0 warpgroups: dV = acc0; set 1 warpgroups: dK = scale * acc1; column half c each
+        constexpr int HALF = DH / 2;
+        mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
+        tc_fence_after();
+        uint32_t acc[HALF];
+        tmem_ld_cols<HALF>(lane_base + (g == 0 ? Cfg::ACC0 : Cfg::ACC1) + c * HALF, acc);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
         if (row < s.R) {
           const float mul = g == 0 ? 1.f : s.scale;
-          __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell;
+          __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell + c * HALF;
 #pragma unroll
-          for (int k = 0; k < DH / 8; ++k) {
+          for (int k = 0; k < HALF / 8; ++k) {
             float f[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) f[e] = row < it.n ? __uint_as_float(acc[8 * k + e]) * mul : 0.f;
@@ -435,7 +448,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 10) tmem_dealloc(tmem, Cfg::COLS);
+  if (warp == kScoreWarps + 1) tmem_dealloc(tmem, Cfg::COLS);
 }
 
 template <int DH>

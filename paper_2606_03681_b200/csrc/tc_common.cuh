@@ -58,7 +58,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait<HINT>(bar, parity)) return;
   uint32_t spins = 0;
   while (!mbar_try_wait<HINT>(bar, parity)) {
-    if (++spins > (1u << (HINT ? 22 : 26))) __trap();
+    if (++spins > (1u << (HINT ? 18 : 22))) __trap();
   }
 }
 
