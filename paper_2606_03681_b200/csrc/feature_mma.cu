@@ -769,6 +769,10 @@ Plan make_plan(const Shape& s, bool bwd) {
   if (warps > kMaxWarps) warps = kMaxWarps;
   if (warps < 1) warps = 1;
   int rows = (!bwd && s.C <= 32 && s.R >= 2 && stage_bytes(hg, 2) <= target) ? 2 : 1;
+  // backward: a stage should hold at least two tasks per warp (key- and query-stationary tasks of every
+  // (row, head, 16-column tile)), else the per-stage barriers dominate: long_item (C = 21, one head per
+  // stage, 4 warps) 1.15 -> 0.92 ms with two rows per stage (B200 sweep, profiles/r01_s23_feature_sweep.md)
+  if (bwd && rows == 1 && s.R >= 2 && 2 * hg * ((s.C + 15) / 16) < 2 * warps && stage_bytes(hg, 2) <= target) rows = 2;
   rows = env_int("TABATTN_FEAT_ROWS", rows);
   const size_t stg_bytes = (size_t)warps * 16 * (s.dh * 2 + 16);
   int nstage = env_int("TABATTN_FEAT_NSTAGE", 2);
