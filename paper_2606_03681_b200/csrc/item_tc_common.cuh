@@ -1,6 +1,6 @@
 // Shared pieces of the tcgen05 item-axis kernels (item_tc_fwd.cu, item_tc_bwd.cu): the persistent
 // work walker, the shared-memory tail zeroing that enforces the train-only key rule on partially
-// filled tiles, and the UMMA issue helpers for the two contraction shapes the path needs.
+// filled tiles, and the setmaxnreg wrappers.
 #pragma once
 #include "common.cuh"
 #include "tc_common.cuh"
@@ -75,28 +75,6 @@ __device__ __forceinline__ void zero_tail_rows(uint32_t tile_saddr, int first_ro
     asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
   tc::fence_proxy_async_smem();
   __syncwarp();
-}
-
-// D[128 x N] (tmem) = A[128 x DH] * B[N x DH]^T, both K-major tiles as TMA wrote them.
-template <int DH, int N = 128>
-__device__ __forceinline__ void issue_qk(uint32_t d_tmem, uint32_t a_saddr, uint32_t b_saddr) {
-  constexpr int ROWB = DH * 2;
-  constexpr uint32_t idesc = tc::make_idesc_bf16(128, N, false, false);
-#pragma unroll
-  for (int k = 0; k < DH / 16; ++k)
-    tc::mma_ss(d_tmem, tc::make_smem_desc<ROWB>(a_saddr + 32 * k, 16, 8 * ROWB),
-               tc::make_smem_desc<ROWB>(b_saddr + 32 * k, 16, 8 * ROWB), idesc, k > 0);
-}
-
-// D[128 x DH] (tmem) (+)= A[128 x KR] (bf16 in tmem, KR/2 columns) * B[KR x DH] (MN-major smem tile).
-template <int DH, int KR = 128>
-__device__ __forceinline__ void issue_pv(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_saddr, bool accumulate) {
-  constexpr int ROWB = DH * 2;
-  constexpr uint32_t idesc = tc::make_idesc_bf16(128, DH, false, true);
-#pragma unroll
-  for (int kk = 0; kk < KR / 16; ++kk)
-    tc::mma_ts(d_tmem, a_tmem + 8 * kk, tc::make_smem_desc<ROWB>(b_saddr + kk * 16 * ROWB, 16, 8 * ROWB), idesc,
-               (accumulate || kk > 0) ? 1u : 0u);
 }
 
 template <int N>

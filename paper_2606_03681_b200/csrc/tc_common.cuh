@@ -58,20 +58,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait<HINT>(bar, parity)) return;
   uint32_t spins = 0;
   while (!mbar_try_wait<HINT>(bar, parity)) {
-    if (++spins > (1u << (HINT ? 18 : 22))) __trap();
+    if (++spins > (1u << (HINT ? 18 : 24))) __trap();
   }
-}
-
-// Wait loop entirely inside one asm statement (no C++-level divergent loop around the issue code).
-__device__ __forceinline__ void mbar_wait_asm(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_LOOP_%=;\n\t"
-      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity), "r"(20000u)
-      : "memory");
 }
 
 // ---- proxies / fences ------------------------------------------------------------------------------
@@ -131,32 +119,6 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, bool a_mn, 
 }
 
 // ---- MMA ---------------------------------------------------------------------------------------------
-// D[tmem] (+)= A[smem] * B[smem]
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                       uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
-      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-// D[tmem] (+)= A[tmem] * B[smem]
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc,
-                                       uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
-      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-// mbarrier arrive when all tcgen05 ops issued so far by this thread have completed
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
-               : "memory");
-}
-
 // ---- warp-convergent issue: every lane of the issuing warp executes these with identical operands;
 // elect.sync picks the one lane that issues.  Keeping the caller's control flow convergent lets ptxas
 // hold descriptors and addresses in uniform registers (no per-lane ELECT/R2UR.BROADCAST replay loop).
