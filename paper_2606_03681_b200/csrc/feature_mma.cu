@@ -259,10 +259,16 @@ __device__ __forceinline__ void stsm4(uint32_t addr, uint32_t r0, uint32_t r1, u
 // row, round to bf16, transpose through the warp's staging tile (stmatrix), and write full 16-byte
 // vectors to the cells (row r of the unit, compacted columns v0..v0+15, head h) of a [B,R,C,H,dh] tensor.
 // `dst_row` points at (table row, column 0, head h); cells of one row are d2 bytes apart.
-template <int DH>
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+
+// IDENT: all columns of the table are valid, slot v is column v (no vcol lookup).
+template <int DH, bool IDENT>
 __device__ __forceinline__ void write_tile(uint32_t stg, const float (&acc)[DH / 8][4], float mul0, float mul1,
-                                           unsigned char* dst_row, uint32_t d2, int v0, int Cv, bool identity,
-                                           const unsigned char* vcol) {
+                                           unsigned char* dst_row, uint32_t d2, int v0, int Cv, uint32_t vcol_s) {
   constexpr int SSTR = DH * 2 + 16, CH = DH / 8;
   const int lane = threadIdx.x & 31;
   {
@@ -280,7 +286,7 @@ __device__ __forceinline__ void write_tile(uint32_t stg, const float (&acc)[DH /
     const int idx = it * 32 + lane;
     const int row = idx / CH, ch = idx % CH;
     if (v0 + row < Cv) {
-      const uint32_t c = identity ? (uint32_t)(v0 + row) : (uint32_t)vcol[v0 + row];
+      const uint32_t c = IDENT ? (uint32_t)(v0 + row) : lds_u8(vcol_s + v0 + row);
       stg_v4(dst_row + (c * d2 + ch * 16), lds128(stg + row * SSTR + ch * 16));
     }
   }
@@ -294,13 +300,12 @@ struct TaskCtx {
   uint32_t str, d2;          // slot stride, bytes per cell
   float c2, scale;           // scale * log2(e), scale
   int Cv;
-  bool identity;             // all columns valid: slot v is column v
-  const unsigned char* vcol;
+  uint32_t vcol_s;           // shared address of the slot -> column table of the stage
 };
 
 // ---- forward task: one warp, 16 query cells (slots v0..v0+15) of one (row, head) ------------------------
 // sQ/sK/sV: shared byte addresses of the slots at (row r of the unit, slot 0, this head).
-template <int DH>
+template <int DH, bool IDENT>
 __device__ __forceinline__ void fwd_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, int v0,
                                          unsigned char* O_row, float* __restrict__ LSE_row) {
   constexpr int KS = DH / 16, NT = DH / 8;
@@ -380,16 +385,19 @@ __device__ __forceinline__ void fwd_task(const TaskCtx& x, uint32_t sQ, uint32_t
   }
   l0 = quad_sum(l0);
   l1 = quad_sum(l1);
-  if (t == 0) {
-    if (v0 + g < Cv) LSE_row[x.identity ? v0 + g : x.vcol[v0 + g]] = (m0 + log2f(l0)) * kLn2;
-    if (v0 + g + 8 < Cv) LSE_row[x.identity ? v0 + g + 8 : x.vcol[v0 + g + 8]] = (m1 + log2f(l1)) * kLn2;
+  if (t < 2) {   // lane t = 0 stores row g, lane t = 1 row g + 8 (every lane of the quad holds both sums)
+    const int rr = v0 + g + 8 * t;
+    if (rr < Cv) {
+      const float lsel = t ? l1 : l0, msel = t ? m1 : m0;
+      LSE_row[IDENT ? (uint32_t)rr : lds_u8(x.vcol_s + rr)] = (msel + log2f(lsel)) * kLn2;
+    }
   }
-  write_tile<DH>(x.stg, o, 1.f / l0, 1.f / l1, O_row, x.d2, v0, Cv, x.identity, x.vcol);
+  write_tile<DH, IDENT>(x.stg, o, 1.f / l0, 1.f / l1, O_row, x.d2, v0, Cv, x.vcol_s);
 }
 
 // ---- backward, key-stationary task: 16 key cells (slots j0..j0+15) of one (row, head) -> dV, dK -----------
 // sL / sD: this (row, head)'s lse*log2e and D vectors, indexed by column slot.
-template <int DH>
+template <int DH, bool IDENT>
 __device__ __forceinline__ void bwd_key_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, uint32_t sG,
                                              const float* sL, const float* sD, int j0, unsigned char* dK_row,
                                              unsigned char* dV_row) {
@@ -459,12 +467,12 @@ __device__ __forceinline__ void bwd_key_task(const TaskCtx& x, uint32_t sQ, uint
       }
     }
   }
-  write_tile<DH>(x.stg, dv, 1.f, 1.f, dV_row, x.d2, j0, Cv, x.identity, x.vcol);
-  write_tile<DH>(x.stg, dk, x.scale, x.scale, dK_row, x.d2, j0, Cv, x.identity, x.vcol);
+  write_tile<DH, IDENT>(x.stg, dv, 1.f, 1.f, dV_row, x.d2, j0, Cv, x.vcol_s);
+  write_tile<DH, IDENT>(x.stg, dk, x.scale, x.scale, dK_row, x.d2, j0, Cv, x.vcol_s);
 }
 
 // ---- backward, query-stationary task: 16 query cells (slots i0..i0+15) of one (row, head) -> dQ -----------
-template <int DH>
+template <int DH, bool IDENT>
 __device__ __forceinline__ void bwd_query_task(const TaskCtx& x, uint32_t sQ, uint32_t sK, uint32_t sV, uint32_t sG,
                                                const float* sL, const float* sD, int i0, unsigned char* dQ_row) {
   constexpr int KS = DH / 16, NT = DH / 8;
@@ -524,7 +532,7 @@ __device__ __forceinline__ void bwd_query_task(const TaskCtx& x, uint32_t sQ, ui
       }
     }
   }
-  write_tile<DH>(x.stg, dq, x.scale, x.scale, dQ_row, x.d2, i0, Cv, x.identity, x.vcol);
+  write_tile<DH, IDENT>(x.stg, dq, x.scale, x.scale, dQ_row, x.d2, i0, Cv, x.vcol_s);
 }
 
 // ---- kernels -------------------------------------------------------------------------------------------------
@@ -595,17 +603,26 @@ __global__ void __launch_bounds__(kMaxWarps * 32) feature_fwd_mma_kernel(const _
     const uint32_t stage = sbase + p.stage0 + buf * p.stage_bytes;
     const unsigned char* sp = smem + p.stage0 + buf * p.stage_bytes;
     x.Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
-    x.vcol = sp + p.off_vcol;
-    x.identity = x.Cv == s.C;
+    x.vcol_s = stage + p.off_vcol;
+    const bool identity = x.Cv == s.C;
     const int MT = (x.Cv + 15) >> 4;
+    // 64-bit bases once per stage, 32-bit offsets per task
     const size_t row0 = (size_t)cu.b * s.R + cu.r0;
+    unsigned char* O_st = O + row0 * s.C * x.d2 + (size_t)cu.hgi * p.hg * DH * 2;
+    float* LSE_st = LSE + (row0 * s.H + (size_t)cu.hgi * p.hg) * s.C;
+    const uint32_t o_row = s.C * x.d2, l_row = s.H * s.C;
     TaskIt it{warp, 0, 0};
     if (MT > 0) {
       for (it.carry(MT, p.hg); it.r < cu.nrows; it.mt += nwarps, it.carry(MT, p.hg)) {
         const uint32_t off = (uint32_t)(it.r * x.Cv) * p.slot_stride + it.hl * DH * 2;
-        const int h = cu.hgi * p.hg + it.hl;
-        fwd_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off, it.mt * 16,
-                     O + (row0 + it.r) * s.C * x.d2 + h * DH * 2, LSE + ((row0 + it.r) * s.H + h) * s.C);
+        unsigned char* O_row = O_st + (it.r * o_row + it.hl * DH * 2);
+        float* LSE_row = LSE_st + (it.r * l_row + it.hl * s.C);
+        if (identity)
+          fwd_task<DH, true>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off, it.mt * 16,
+                             O_row, LSE_row);
+        else
+          fwd_task<DH, false>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off, it.mt * 16,
+                              O_row, LSE_row);
       }
     }
     buf = buf + 1 == NSTAGE ? 0 : buf + 1;
@@ -664,8 +681,8 @@ __global__ void __launch_bounds__(kMaxWarps * 32) feature_bwd_mma_kernel(
     const uint32_t stage = sbase + p.stage0 + buf * p.stage_bytes;
     unsigned char* sp = smem + p.stage0 + buf * p.stage_bytes;
     x.Cv = *reinterpret_cast<const int*>(sp + p.off_cv);
-    x.vcol = sp + p.off_vcol;
-    x.identity = x.Cv == s.C;
+    x.vcol_s = stage + p.off_vcol;
+    const bool identity = x.Cv == s.C;
     const int Cv = x.Cv;
     float* sL = reinterpret_cast<float*>(sp + p.off_lse);
     float* sD = reinterpret_cast<float*>(sp + p.off_D);
@@ -712,12 +729,14 @@ __global__ void __launch_bounds__(kMaxWarps * 32) feature_bwd_mma_kernel(
       const float* L = sL + (it.r * p.hg + it.hl) * p.Cp;
       const float* D = sD + (it.r * p.hg + it.hl) * p.Cp;
       const size_t goff = (rowcell0 + (size_t)it.r * s.C) * x.d2 + (cu.hgi * p.hg + it.hl) * DH * 2;
-      if (key_task)
-        bwd_key_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
-                         stage + 3 * p.slot_bytes + off, L, D, it.mt * 16, dK + goff, dV + goff);
-      else
-        bwd_query_task<DH>(x, stage + off, stage + p.slot_bytes + off, stage + 2 * p.slot_bytes + off,
-                           stage + 3 * p.slot_bytes + off, L, D, it.mt * 16, dQ + goff);
+      const uint32_t sq = stage + off, sk = sq + p.slot_bytes, sv = sk + p.slot_bytes, sg = sv + p.slot_bytes;
+      if (key_task) {
+        if (identity) bwd_key_task<DH, true>(x, sq, sk, sv, sg, L, D, it.mt * 16, dK + goff, dV + goff);
+        else bwd_key_task<DH, false>(x, sq, sk, sv, sg, L, D, it.mt * 16, dK + goff, dV + goff);
+      } else {
+        if (identity) bwd_query_task<DH, true>(x, sq, sk, sv, sg, L, D, it.mt * 16, dQ + goff);
+        else bwd_query_task<DH, false>(x, sq, sk, sv, sg, L, D, it.mt * 16, dQ + goff);
+      }
       it.mt += nwarps;
     }
     buf = buf + 1 == NSTAGE ? 0 : buf + 1;
