@@ -76,8 +76,11 @@ struct Item {
 template <int MODE>
 __device__ __forceinline__ Item decode_item(const Shape& s, int w, int bps) {
   Item it;
-  it.blk = w % bps;
   const int rest = w / bps;
+  // MODE_DKV: key blocks >= n_train are invalid (skipped).  With blk = w % bps a CTA (w = x + 148 k) would see
+  // only a few residues of blk -- at bps = 8, n = 768 half of the CTAs get 50 % invalid items and the others
+  // none (1.33x imbalance, base) -- so the block index is rotated by the sequence index.
+  it.blk = MODE == MODE_DKV ? (w % bps + rest) % bps : w % bps;
   it.h = rest % s.H;
   const int bc = rest / s.H;
   it.b = bc / s.C;
