@@ -61,6 +61,11 @@ EDGE = [
     ("wide_C", 1, 9, 128, 1, 32, 5),          # largest feature-axis length
     ("c17", 2, 40, 17, 2, 32, 30),
     ("c33_dh64", 1, 24, 33, 2, 64, 17),
+    # more work items than SMs (several items per persistent CTA), key-block rotation of the dK/dV pass with
+    # a non-power-of-two block count, last 64-key chunk split 32 + 12 / 14 + 0 between the column halves
+    ("multi_item_dh32", 3, 700, 5, 2, 32, 300),
+    ("multi_item_dh64", 4, 520, 5, 2, 64, 270),
+    ("dh16_multi_chunk", 2, 300, 3, 2, 16, 200),
 ]
 
 
