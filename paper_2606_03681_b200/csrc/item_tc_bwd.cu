@@ -335,7 +335,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         nlse2 = __ldg(lse2_ws + seq + row);
         Drow = __ldg(D_ws + seq + row);
       }
-      const uint64_t cc = f2pack(c2, c2), nl = f2pack(nlse2, nlse2), dd = f2pack(Drow, Drow);
+      const uint64_t nl = f2pack(nlse2, nlse2), dd = f2pack(Drow, Drow);
       const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
@@ -347,7 +347,14 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(b_s_empty);
+        // Release the set's S/dP columns.  At dh = 64 the next S/dP MMAs (256 tensor clk) are on the critical
+        // chain, so the arithmetic is made to depend on the arrive (mbar_arrive_then: long_item bwd 7.52 ->
+        // 7.28 ms); at dh <= 32 they are not, and letting ptxas overlap the arithmetic on S with the dP load
+        // is worth more (base bwd 1.56 against 1.63 ms).
+        float c2d = c2;
+        if constexpr (DH >= 64) c2d = mbar_arrive_then(b_s_empty, lane == 0, c2);
+        else if (lane == 0) mbar_arrive(b_s_empty);
+        const uint64_t cc = f2pack(c2d, c2d);
         uint32_t pds[16], pp[16];
         if (MODE == MODE_DQ) {
           // P = 2^(S*c2 - lse2), dS = P o (dP - D) on packed fp32 pairs

@@ -179,6 +179,25 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
                : "r"(taddr)
                : "memory");
 }
+// mbarrier arrive (by the lanes with do_arrive != 0) whose completion the returned value depends on: `carry`
+// comes back unchanged, but through an instruction that consumes the arrive's state token, so arithmetic that
+// uses the result cannot be scheduled above the arrive.  Without this ptxas sinks the arrive that releases a
+// TMEM buffer under most of the arithmetic on the loaded registers (it has no data dependency on it), which
+// delays the next MMAs into that buffer by most of a chunk's compute time (profiles/r01_s27_final.md).
+__device__ __forceinline__ float mbar_arrive_then(uint32_t bar, uint32_t do_arrive, float carry) {
+  asm volatile(
+      "{\n\t.reg .b64 st;\n\t.reg .b32 lo, hi;\n\t.reg .pred q, p;\n\t"
+      "setp.ne.b32 q, %2, 0;\n\t"
+      "mov.b64 st, 0;\n\t"
+      "@q mbarrier.arrive.shared::cta.b64 st, [%1];\n\t"
+      "mov.b64 {lo, hi}, st;\n\t"
+      "setp.eq.u32 p, hi, 0xdeadbeef;\n\t"          // never true for a real barrier state; adding +0 is harmless
+      "@p add.f32 %0, %0, 0f00000000;\n\t}"
+      : "+f"(carry)
+      : "r"(bar), "r"(do_arrive)
+      : "memory");
+  return carry;
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // N columns (16, 32 or 64) starting at taddr, then wait.
 template <int N>
