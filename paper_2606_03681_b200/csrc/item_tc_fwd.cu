@@ -86,7 +86,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
   const uint32_t tmem = tmem_slot;
 
   if (warp >= 8) {
-    setmaxnreg_dec<80>();
+    setmaxnreg_dec<64>();
     if (warp == 8) {
       // ------------------------------------------------------------------ TMA producer
       if (lane == 0) {
@@ -213,7 +213,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     }
   } else {
     // -------------------------------------------------------------------- softmax warpgroups
-    setmaxnreg_inc<208>();
+    setmaxnreg_inc<216>();
     const int t = warp >> 2;                  // query tile of this warpgroup
     const int r = threadIdx.x & 127;          // row inside the tile = TMEM lane
     const uint32_t lane_base = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
