@@ -157,3 +157,33 @@ SCALED = [
 @pytest.mark.parametrize("name,kw", SCALED, ids=[s[0] for s in SCALED])
 def test_scaled_configs(name, kw, axis):
     _run_case(get_config(name).scaled(**kw), axis, poison=True)
+
+
+# ---- the pipelined host path (layer_fwd_bwd_host) must give the device path's bits -------------------
+def test_host_pipeline_matches_device_path():
+    import torch
+    import paper_2606_03681_b200 as tab
+    cfg = get_config("ragged").scaled(B=5, R=200, ragged_n_train=(40, 150))
+    nt_h, cv_h = draw_structure(cfg)
+    dev = torch.device("cuda", 0)
+    nt = torch.from_numpy(nt_h).to(dev)
+    cv = torch.from_numpy(cv_h).to(dev) if cv_h is not None else None
+    L = {ax: make_call_inputs(cfg, ax, 0, device=dev) for ax in ("feature", "item")}
+    ref_buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
+    tab.layer_fwd_bwd(L["feature"], L["item"], nt, cv, ref_buf, nt_h)
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (ref_buf.O_f, ref_buf.O_i) + ref_buf.grads_f + ref_buf.grads_i]
+    host = {ax: {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in L[ax].items()}
+            for ax in L}
+    stage = {ax: {k: torch.zeros_like(v) for k, v in L[ax].items()} for ax in L}
+    out_host = [torch.zeros(want[0].shape, dtype=torch.bfloat16, pin_memory=True) for _ in range(8)]
+    buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
+    for groups in (1, 3, 4):          # 5 tables: uneven groups too
+        for t in out_host:
+            t.zero_()
+        h2d, d2h = tab.layer_fwd_bwd_host(host["feature"], host["item"], stage["feature"], stage["item"],
+                                          out_host, nt, cv, buf, nt_h, groups=groups)
+        torch.cuda.synchronize()
+        assert h2d == 8 * want[0].numel() * 2 and d2h == 8 * want[0].numel() * 2
+        for got, w in zip(out_host, want):
+            assert torch.equal(got.view(torch.int16), w.cpu().view(torch.int16)), "groups=%d" % groups
