@@ -187,3 +187,37 @@ def test_host_pipeline_matches_device_path():
         assert h2d == 8 * want[0].numel() * 2 and d2h == 8 * want[0].numel() * 2
         for got, w in zip(out_host, want):
             assert torch.equal(got.view(torch.int16), w.cpu().view(torch.int16)), "groups=%d" % groups
+
+
+# ---- the library only enqueues on the caller's stream: the four calls can be captured in a CUDA graph ----
+def test_layer_is_graph_capturable():
+    import torch
+    import paper_2606_03681_b200 as tab
+    cfg = get_config("base").scaled(B=2, R=300, n_train=200)
+    nt_h, cv_h = draw_structure(cfg)
+    dev = torch.device("cuda", 0)
+    nt = torch.from_numpy(nt_h).to(dev)
+    cv = torch.from_numpy(cv_h).to(dev) if cv_h is not None else None
+    L = {ax: make_call_inputs(cfg, ax, 0, device=dev) for ax in ("feature", "item")}
+    buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
+    tab.layer_fwd_bwd(L["feature"], L["item"], nt, cv, buf, nt_h)      # eager (also warms up lazy init)
+    torch.cuda.synchronize()
+    outs = (buf.O_f, buf.O_i) + buf.grads_f + buf.grads_i
+    want = [t.clone() for t in outs]
+    for t in outs:
+        t.zero_()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            tab.layer_fwd_bwd(L["feature"], L["item"], nt, cv, buf, nt_h)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    for rep in range(2):
+        for t in outs:
+            t.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for got, w in zip(outs, want):
+            assert torch.equal(got.view(torch.int16), w.view(torch.int16)), "replay %d" % rep
