@@ -887,8 +887,25 @@ Plan make_plan(const Shape& s, bool bwd) {
     --hg;
     while (hg > 1 && s.H % hg != 0) --hg;
   }
+  int warps = s.C <= 16 ? 2 : 4;
+  int nstage = env_int("TABATTN_FEAT_NSTAGE", 2);
+  if (bwd) {
+    // The backward needs >= 12 resident warps per SM to cover its latencies (B200 sweep,
+    // profiles/r01_s23_feature_sweep.md): ragged (C = 51) 1.63 -> 1.41 ms with one head per stage (4 CTAs per SM
+    // instead of 2), feature_heavy (C = 101, already one head per stage) 0.94 -> 0.84 ms with 6 warps per CTA.
+    auto ctas = [&](int hg_, int warps_) {
+      const size_t smem = (size_t)warps_ * 16 * (s.dh * 2 + 16) + (size_t)nstage * stage_bytes(hg_, 1);
+      int c = (int)(kSmemPerSM / (smem + 1024));
+      const int by_regs = 65536 / (warps_ * 32 * (s.dh >= 64 ? 168 : 128));
+      c = c < by_regs ? c : by_regs;
+      return c < 1 ? 1 : (c > 8 ? 8 : c);
+    };
+    if (ctas(hg, warps) * warps < 12 && hg > 1 && ctas(1, warps) > ctas(hg, warps)) hg = 1;
+    const int c = ctas(hg, warps);
+    if (c * warps < 12) warps = (12 + c - 1) / c;
+  }
   hg = env_int("TABATTN_FEAT_HG", hg);
-  int warps = env_int("TABATTN_FEAT_WARPS", s.C <= 16 ? 2 : 4);
+  warps = env_int("TABATTN_FEAT_WARPS", warps);
   if (warps > kMaxWarps) warps = kMaxWarps;
   if (warps < 1) warps = 1;
   int rows = (!bwd && s.C <= 32 && s.R >= 2 && stage_bytes(hg, 2) <= target) ? 2 : 1;
@@ -898,7 +915,6 @@ Plan make_plan(const Shape& s, bool bwd) {
   if (bwd && rows == 1 && s.R >= 2 && 2 * hg * ((s.C + 15) / 16) < 2 * warps && stage_bytes(hg, 2) <= target) rows = 2;
   rows = env_int("TABATTN_FEAT_ROWS", rows);
   const size_t stg_bytes = (size_t)warps * 16 * (s.dh * 2 + 16);
-  int nstage = env_int("TABATTN_FEAT_NSTAGE", 2);
   p.hg = hg;
   p.nhg = s.H / hg;
   p.rows = rows;
