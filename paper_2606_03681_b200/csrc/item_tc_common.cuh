@@ -19,27 +19,72 @@ __device__ __forceinline__ int clamp_n(const Shape& s, int b) { return max(1, mi
 // invalid columns are skipped here (the zero-fill of their outputs is done by the epilogue warps).
 // `tiles` = number of 128-row tiles of the looped axis; `t` counts tiles over the CTA's lifetime
 // and `k` counts valid items: they index the mbarrier ring phases.
+// Incremental decode of the work items w = blockIdx.x + k * gridDim.x, w = ((b*C + c)*H + h)*bps + blk: the
+// six integer divisions of a direct decode are paid once; next() is ~15 adds/compares with carries.  (At base the
+// items are 6-16 inner tiles long and the direct decode plus the loads that depend on it were ~12 % of the score
+// warps' samples, profiles/r01_s27_final.md.)  seqmod = (sequence index) % bps serves the dK/dV block rotation.
+struct ItemCoord {
+  int w, blk, h, c, b, seqmod;
+  int s_blk, s_h, s_c, s_b, s_seqmod;   // per-step increments (step = gridDim.x items)
+  int bps, H, C;
+  __device__ __forceinline__ void init(const Shape& s, int bps_) {
+    bps = bps_; H = s.H; C = s.C;
+    w = blockIdx.x;
+    blk = w % bps;
+    const int seq = w / bps;
+    h = seq % H;
+    const int bc = seq / H;
+    b = bc / C;
+    c = bc - b * C;
+    seqmod = seq % bps;
+    const int G = gridDim.x, dseq = G / bps;
+    s_blk = G - dseq * bps;
+    s_h = dseq % H;
+    const int dbc = dseq / H;
+    s_b = dbc / C;
+    s_c = dbc - s_b * C;
+    s_seqmod = dseq % bps;
+  }
+  __device__ __forceinline__ void next() {
+    w += gridDim.x;
+    blk += s_blk;
+    const int c0 = blk >= bps;
+    blk -= c0 ? bps : 0;
+    seqmod += s_seqmod + c0;
+    seqmod -= seqmod >= bps ? bps : 0;
+    h += s_h + c0;
+    const int c1 = h >= H;
+    h -= c1 ? H : 0;
+    c += s_c + c1;
+    const int c2 = c >= C;
+    c -= c2 ? C : 0;
+    b += s_b + c2;
+  }
+  __device__ __forceinline__ int bc() const { return b * C + c; }
+  // dK/dV pass: block index rotated by the sequence index (see decode_item)
+  __device__ __forceinline__ int blk_rot() const {
+    const int r = blk + seqmod;
+    return r >= bps ? r - bps : r;
+  }
+};
+
 struct Walker {
-  int w, j, tiles, n, b, c, h, blk;
+  ItemCoord ic;
+  int j, tiles, n, b, c, h, blk;
   uint32_t k, t;
   bool ok;
-  int n_items, bps, chunk;   // items in the launch, 128/256-row blocks per sequence, rows per inner tile
+  int n_items, chunk;        // items in the launch, rows per inner tile
   bool over_keys;            // inner axis = key rows [0, n) (fwd, dQ); else query rows [0, R) (dK/dV)
 
   __device__ __forceinline__ void decode(const Shape& s, bool& valid) {
-    blk = w % bps;
-    const int rest = w / bps;
-    h = rest % s.H;
-    const int bc = rest / s.H;
-    b = bc / s.C;
-    c = bc - b * s.C;
+    blk = ic.blk; h = ic.h; b = ic.b; c = ic.c;
     n = clamp_n(s, b);
-    valid = (!s.col_valid || __ldg(s.col_valid + bc) != 0) && (over_keys || blk * kTileRows < n);
+    valid = (!s.col_valid || __ldg(s.col_valid + ic.bc()) != 0) && (over_keys || blk * kTileRows < n);
     tiles = ((over_keys ? n : s.R) + chunk - 1) / chunk;
   }
   __device__ __forceinline__ void seek(const Shape& s) {
     ok = false;
-    while (w < n_items) {
+    while (ic.w < n_items) {
       bool valid;
       decode(s, valid);
       if (valid) {
@@ -47,18 +92,19 @@ struct Walker {
         ok = true;
         return;
       }
-      w += gridDim.x;
+      ic.next();
     }
   }
   __device__ __forceinline__ void init(const Shape& s, int n_items_, int bps_, int chunk_, bool over_keys_) {
-    n_items = n_items_; bps = bps_; chunk = chunk_; over_keys = over_keys_;
-    w = blockIdx.x; k = 0; t = 0;
+    n_items = n_items_; chunk = chunk_; over_keys = over_keys_;
+    ic.init(s, bps_);
+    k = 0; t = 0;
     seek(s);
   }
   __device__ __forceinline__ void next(const Shape& s) {
     ++t;
     if (++j == tiles) {
-      w += gridDim.x;
+      ic.next();
       ++k;
       seek(s);
     }

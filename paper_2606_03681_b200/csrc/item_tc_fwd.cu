@@ -125,12 +125,13 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       // builds of this kernel (profiles/r01_s7_full.md, r01_s14_item.md); three warps in parallel do not.
       constexpr uint32_t TILE16 = TILE >> 4;
       uint32_t st = 0, ph = 0, par = 0, j = 0, tiles = 0, k = 0;
-      int w = blockIdx.x, n = 0;
+      int n = 0;
+      ItemCoord ic;
+      ic.init(s, blocks_per_seq);
       auto seek = [&]() {
-        for (; w < n_items; w += gridDim.x) {
-          const int bc = w / (blocks_per_seq * s.H);
-          if (s.col_valid && __ldg(s.col_valid + bc) == 0) continue;
-          n = clamp_n(s, bc / s.C);
+        for (; ic.w < n_items; ic.next()) {
+          if (s.col_valid && __ldg(s.col_valid + ic.bc()) == 0) continue;
+          n = clamp_n(s, ic.b);
           tiles = (uint32_t)(n + kTileRows - 1) / kTileRows;
           return true;
         }
@@ -180,7 +181,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           if (++j == tiles) {
             j = 0;
             ++k;
-            w += gridDim.x;
+            ic.next();
             ok = seek();
           }
         }
@@ -205,7 +206,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           if (++st == ST) { st = 0; ph ^= 1; }
           if (++j == tiles) {
             j = 0;
-            w += gridDim.x;
+            ic.next();
             ok = seek();
           }
         }
@@ -224,10 +225,10 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const float c2 = s.scale * kLog2e;
     const int d = s.H * DH;
     uint32_t g = 0;  // tiles processed by this CTA so far
-    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      Walker it;
-      it.n_items = n_items; it.bps = blocks_per_seq; it.chunk = kTileRows; it.over_keys = true;
-      it.w = w;
+    Walker it;
+    it.n_items = n_items; it.chunk = kTileRows; it.over_keys = true;
+    it.ic.init(s, blocks_per_seq);
+    for (; it.ic.w < n_items; it.ic.next()) {
       bool valid;
       it.decode(s, valid);
       const int row = it.blk * 2 * kTileRows + t * kTileRows + r;
