@@ -74,7 +74,7 @@ struct Item {
 };
 
 template <int MODE>
-__device__ __forceinline__ Item decode_item(const Shape& s, int w, int bps) {
+__device__ __forceinline__ Item decode_item(const Shape& s, const Meta& meta, int w, int bps) {
   Item it;
   const int rest = w / bps;
   // MODE_DKV: key blocks >= n_train are invalid (skipped).  With blk = w % bps a CTA (w = x + 148 k) would see
@@ -85,8 +85,8 @@ __device__ __forceinline__ Item decode_item(const Shape& s, int w, int bps) {
   const int bc = rest / s.H;
   it.b = bc / s.C;
   it.c = bc - it.b * s.C;
-  it.n = clamp_n(s, it.b);
-  it.valid = (!s.col_valid || __ldg(s.col_valid + bc) != 0) && (MODE == MODE_DQ || it.blk * kTileRows < it.n);
+  it.n = meta.n(s, it.b);
+  it.valid = meta.cv(s, bc) && (MODE == MODE_DQ || it.blk * kTileRows < it.n);
   it.chunks = ((MODE == MODE_DQ ? it.n : s.R) + kChunk - 1) / kChunk;
   return it;
 }
@@ -159,6 +159,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   __shared__ uint64_t bar_a_full[2], bar_a_empty[2], bar_b_full[ST], bar_b_empty[ST];
   __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_p_empty[2], bar_acc_full, bar_acc_free;
   __shared__ uint32_t tmem_slot;
+  __shared__ int32_t s_ntrain[kMetaTabs];
+  __shared__ uint8_t s_colvalid[kMetaCells];
+  Meta meta;
+  meta.fill(s, s_ntrain, s_colvalid);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // provably warp-uniform
   if (warp == kScoreWarps + 1) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
@@ -197,7 +201,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       tma_prefetch_desc(&mapB2);
       uint32_t t = 0, k = 0;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-        const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+        const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
         if (!it.valid) continue;
         const uint32_t ab = k & 1, a_full = smem_u32(&bar_a_full[ab]);
         mbar_wait<true>(smem_u32(&bar_a_empty[ab]), ((k >> 1) & 1) ^ 1);
@@ -232,7 +236,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                    b_s_empty = smem_u32(&bar_s_empty[0]);
     uint32_t t = 0, k = 0, st = 0, ph = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
       mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
@@ -275,7 +279,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                    b_b_empty = smem_u32(&bar_b_empty[0]);
     uint32_t t = 0, k = 0, st = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
       if (!it.valid) continue;
       mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
       for (int j = 0; j < it.chunks; ++j, ++t) {
@@ -311,7 +315,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     uint32_t kitem = 0;   // valid items seen
     uint32_t tbase = 0;   // chunks of all previous valid items (ring position)
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, w, blocks_per_seq);
+      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
       const int row = it.blk * kTileRows + r;
       const size_t cell = (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
       const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
