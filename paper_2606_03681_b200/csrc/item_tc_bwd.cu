@@ -314,6 +314,59 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     const float c2 = s.scale * kLog2e;
     uint32_t kitem = 0;   // valid items seen
     uint32_t tbase = 0;   // chunks of all previous valid items (ring position)
+    // ---- epilogue of one item (accumulators -> global), as a deferred step: it runs after the warpgroup's first
+    // chunk of the NEXT item, so that the wait for the item's last accumulation MMAs (bar_acc_full) is covered
+    // by that chunk's arithmetic instead of idling at every item boundary.
+    auto epilogue = [&](size_t e_cell, int e_row, int e_n, uint32_t e_par) {
+        if (MODE == MODE_DQ) {
+          // the dQ columns of a row are split over the four warpgroups (two at dh = 16: 16-byte stores)
+          constexpr int EPW = DH >= 32 ? 4 : 2, PART = DH / EPW;
+          const int q = g + 2 * c;
+          if (q < EPW) {
+            mbar_wait(smem_u32(&bar_acc_full), e_par);
+            tc_fence_after();
+            uint32_t acc[PART];
+            tmem_ld_cols<PART>(lane_base + Cfg::ACC0 + q * PART, acc);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
+            if (e_row < s.R) {
+  #pragma unroll
+              for (int k = 0; k < PART / 8; ++k) {
+                float f[8];
+  #pragma unroll
+                for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(acc[8 * k + e]) * s.scale;
+                stg_v4(out0 + e_cell + q * PART + 8 * k, pack8(f));
+              }
+            }
+          }
+        } else {
+          // set 0 warpgroups: dV = acc0; set 1 warpgroups: dK = scale * acc1; column half c each
+          constexpr int HALF = DH / 2;
+          mbar_wait(smem_u32(&bar_acc_full), e_par);
+          tc_fence_after();
+          uint32_t acc[HALF];
+          tmem_ld_cols<HALF>(lane_base + (g == 0 ? Cfg::ACC0 : Cfg::ACC1) + c * HALF, acc);
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
+          if (e_row < s.R) {
+            const float mul = g == 0 ? 1.f : s.scale;
+            __nv_bfloat16* dst = (g == 0 ? out0 : out1) + e_cell + c * HALF;
+  #pragma unroll
+            for (int k = 0; k < HALF / 8; ++k) {
+              float f[8];
+  #pragma unroll
+              for (int e = 0; e < 8; ++e) f[e] = e_row < e_n ? __uint_as_float(acc[8 * k + e]) * mul : 0.f;
+              stg_v4(dst + 8 * k, pack8(f));
+            }
+          }
+        }
+    };
+    bool pend = false;
+    size_t p_cell = 0;
+    int p_row = 0, p_n = 0;
+    uint32_t p_par = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
       const int row = it.blk * kTileRows + r;
@@ -410,55 +463,18 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(b_p_full);
-      }
-      // ---- epilogue ---------------------------------------------------------------------------------
-      if (MODE == MODE_DQ) {
-        // the dQ columns of a row are split over the four warpgroups (two at dh = 16: 16-byte stores)
-        constexpr int EPW = DH >= 32 ? 4 : 2, PART = DH / EPW;
-        const int q = g + 2 * c;
-        if (q < EPW) {
-          mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
-          tc_fence_after();
-          uint32_t acc[PART];
-          tmem_ld_cols<PART>(lane_base + Cfg::ACC0 + q * PART, acc);
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
-          if (row < s.R) {
-#pragma unroll
-            for (int k = 0; k < PART / 8; ++k) {
-              float f[8];
-#pragma unroll
-              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(acc[8 * k + e]) * s.scale;
-              stg_v4(out0 + cell + q * PART + 8 * k, pack8(f));
-            }
-          }
-        }
-      } else {
-        // set 0 warpgroups: dV = acc0; set 1 warpgroups: dK = scale * acc1; column half c each
-        constexpr int HALF = DH / 2;
-        mbar_wait(smem_u32(&bar_acc_full), kitem & 1);
-        tc_fence_after();
-        uint32_t acc[HALF];
-        tmem_ld_cols<HALF>(lane_base + (g == 0 ? Cfg::ACC0 : Cfg::ACC1) + c * HALF, acc);
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free));
-        if (row < s.R) {
-          const float mul = g == 0 ? 1.f : s.scale;
-          __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell + c * HALF;
-#pragma unroll
-          for (int k = 0; k < HALF / 8; ++k) {
-            float f[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = row < it.n ? __uint_as_float(acc[8 * k + e]) * mul : 0.f;
-            stg_v4(dst + 8 * k, pack8(f));
-          }
+        if (pend) {
+          epilogue(p_cell, p_row, p_n, p_par);
+          pend = false;
         }
       }
+      // the epilogue of this item is deferred (see `epilogue` above)
+      if (pend) epilogue(p_cell, p_row, p_n, p_par);   // (no chunk of the item was ours)
+      pend = true; p_cell = cell; p_row = row; p_n = it.n; p_par = kitem & 1;
       ++kitem;
       tbase += chunks;
     }
+    if (pend) epilogue(p_cell, p_row, p_n, p_par);
   }
   tc_fence_before();
   __syncthreads();
