@@ -37,9 +37,10 @@ struct FwdCfg {
   // TMEM columns
   static constexpr int S0 = 0, P0 = 256, O0 = 384, COLS = 512;
   static_assert(O0 + 2 * DH <= COLS, "TMEM budget");
-  // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2) instead of the MUFU: measured
-  // on B200 (profiles/r01_s14_item.md) +8 % at dh = 32, -1.5 % (2 of 8) to -16 % (5 of 8) at dh = 64
-  static constexpr int POLY_OF_8 = DH >= 64 ? 0 : 2;
+  // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2) instead of the MUFU.  Measured on B200
+  // (profiles/r01_s14_item.md, r01_s42_final.md): 2 of 8 gives +8 % at dh = 32 and +2 % at dh = 64 (after the issue
+  // and item-decode overheads were removed; it was -1.5 % before), larger shares lose at both.
+  static constexpr int POLY_OF_8 = 2;
 };
 
 constexpr int kFwdThreads = 384;
