@@ -38,7 +38,7 @@ struct FwdCfg {
   static constexpr int S0 = 0, P0 = 256, O0 = 384, COLS = 512;
   static_assert(O0 + 2 * DH <= COLS, "TMEM budget");
   // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2) instead of the MUFU.  Measured on B200
-  // (profiles/r01_s14_item.md, r01_s42_final.md): 2 of 8 gives +8 % at dh = 32 and +2 % at dh = 64 (after the issue
+  // (profiles/r01_s14_item.md, r01_s46_final.md): 2 of 8 gives +8 % at dh = 32 and +2 % at dh = 64 (after the issue
   // and item-decode overheads were removed; it was -1.5 % before), larger shares lose at both.
   static constexpr int POLY_OF_8 = 2;
 };
