@@ -66,6 +66,9 @@ EDGE = [
     ("multi_item_dh32", 3, 700, 5, 2, 32, 300),
     ("multi_item_dh64", 4, 520, 5, 2, 64, 270),
     ("dh16_multi_chunk", 2, 300, 3, 2, 16, 200),
+    # B*C = 8960 > 8192 cells: the backward kernels read n_train / col_valid from global memory instead of
+    # their shared-memory copy (item_tc_common.cuh: Meta)
+    ("meta_global_path", 70, 16, 128, 1, 16, 9),
 ]
 
 
