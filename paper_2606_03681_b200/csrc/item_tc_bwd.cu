@@ -55,7 +55,9 @@ struct BwdCfg {
   static constexpr int ROWB = DH * 2;
   static constexpr int TILE_A = kTileRows * ROWB;  // stationary tile
   static constexpr int TILE_B = kChunk * ROWB;     // streamed chunk
-  static constexpr int ST = 6;                     // chunk ring depth
+  // chunk ring depth: as deep as shared memory allows at dh = 64 (8 stages, 196 KB); 16 at dh <= 32 (B200 sweep:
+  // base bwd 1.451 / 1.436 / 1.414 / 1.404 / 1.418 ms at 6 / 8 / 12 / 16 / 20 stages, 1.586 at 4)
+  static constexpr int ST = DH >= 64 ? 8 : 16;
   static constexpr int LD_BYTES = 2 * kChunk * 4;  // per stage: lse2[64], D[64] (MODE_DKV)
   static constexpr int STAGE = 2 * TILE_B;         // bytes of one ring stage (B1, B2)
   static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + 1024;
