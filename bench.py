@@ -320,7 +320,7 @@ def run_ours(args):
         barrier()
         et = max_over_ranks(a.elapsed_time(b) / e_steps, world, dev)
         e2e = {"value": job_value(et, 1, world), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "note": "one layer per step from pinned host buffers, pipelined over 8 table groups (H2D, kernels, D2H on three streams)"}
+               "d2h_bytes_per_step": int(d2h), "note": "one layer per step from pinned host buffers, pipelined over up to 16 table groups (H2D, kernels, D2H on three streams)"}
         del host, stage, out_host
 
     if rank != 0:

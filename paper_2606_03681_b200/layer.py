@@ -64,7 +64,7 @@ class _View:
 
 
 def layer_fwd_bwd_host(feat_host, item_host, feat_dev, item_dev, out_host, n_train, col_valid,
-                       buf: LayerBuffers, n_train_host=None, groups=8):
+                       buf: LayerBuffers, n_train_host=None, groups=16):
     """The same step from pinned host buffers: H2D of the 8 inputs, the four calls, D2H of the
     8 results (O and dQ/dK/dV of both axes) into ``out_host``.  Returns (h2d_bytes, d2h_bytes).
 
