@@ -98,7 +98,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         for (wk.init(s, n_items, blocks_per_seq, kTileRows, true); wk.ok; wk.next(s)) {
           if (wk.j == 0) {
             const int qb = wk.k & 1;
-            mbar_wait(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
+            mbar_wait<true>(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
             mbar_arrive_expect_tx(smem_u32(&bar_q_full[qb]), 2 * TILE);
             const int q0 = wk.blk * 2 * kTileRows;
             tma_load_5d(sQ + (2 * qb) * TILE, &mapQ, smem_u32(&bar_q_full[qb]), 0, wk.h, wk.c, q0, wk.b);
@@ -106,10 +106,10 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                         wk.b);
           }
           const int st = wk.t % ST;
-          mbar_wait(smem_u32(&bar_k_empty[st]), ((wk.t / ST) & 1) ^ 1);
+          mbar_wait<true>(smem_u32(&bar_k_empty[st]), ((wk.t / ST) & 1) ^ 1);
           mbar_arrive_expect_tx(smem_u32(&bar_k_full[st]), TILE);
           tma_load_5d(sK + st * TILE, &mapK, smem_u32(&bar_k_full[st]), 0, wk.h, wk.c, wk.j * kTileRows, wk.b);
-          mbar_wait(smem_u32(&bar_v_empty[st]), ((wk.t / ST) & 1) ^ 1);
+          mbar_wait<true>(smem_u32(&bar_v_empty[st]), ((wk.t / ST) & 1) ^ 1);
           // a partially valid last tile goes through the tail fix (warp 9) before the PV MMAs see it
           const bool tail = wk.j == wk.tiles - 1 && wk.n % kTileRows != 0;
           const uint32_t vbar = tail ? smem_u32(&bar_v_land[st]) : smem_u32(&bar_v_full[st]);
