@@ -1,11 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- dual-axis attention fwd+bwd ms/layer on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config base] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config long_item] [--impl ours|reference]
 
-A "step" is one pass of the whole hot path: feature fwd, item fwd, item bwd,
-feature bwd through the C ABI of libtabattn on one layer of seeded synthetic input (for the
-12-layer Ragged config: all 12 layers, reported per layer).  One JSON line is printed by rank 0.
+A "step" is one pass of the whole hot path over one batch of seeded synthetic
+input, enqueued as a training step would (reading c17): the forward calls (feature fwd, item fwd)
+of every layer of the batch in layer order, then the backward calls (item bwd, feature bwd) in
+reverse order, through the C ABI of libtabattn.  The batch holds `layers_per_step` layers: the
+config's own layer count (12 for Ragged, 1 otherwise) times a repeat factor chosen so that the K
+timed steps last at least --min-region seconds (a sustained-clock number); `value` is ms per
+layer.  The default config is long_item, the one SURVEY.md §8(d) grades the tensor-core bar on;
+the other timed configs (base, feature_heavy, ragged) are measured in the same run under
+`configs`.  One JSON line is printed by rank 0.
 ``--impl reference`` times the fp64 CPU oracle (oracle/) on a bounded sample of the same
 workload instead; it is the only other place this file executes anything under oracle/
 (besides the cpu_baseline leg at N=1).
@@ -28,6 +34,8 @@ from workloads import get_config, draw_structure, make_call_inputs  # noqa: E402
 METRIC = "dual-axis attn fwd+bwd ms/layer"
 UNIT = "ms/layer"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+NOMINAL_PEAKS = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}     # BASELINE.json north_star's figures
+SECONDARY = ("base", "feature_heavy", "ragged")               # timed beside the headline config
 
 
 # ---- algorithmic work (SURVEY.md §8(d) "Algorithmic work per unit") ----------
@@ -76,7 +84,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -114,7 +122,7 @@ class ClockSampler:
 
 
 # ---- the oracle on a bounded sample (cpu_baseline leg and --impl reference) ------------------------
-def oracle_sample_ms_per_layer(cfg, budget_s=12.0):
+def oracle_sample_ms_per_layer(cfg, budget_s=12.0, nthreads=0):
     """Time the fp64 oracle, as it stands, on a bounded seeded sample of one layer of ``cfg`` and
     extrapolate to ms/layer by algorithmic flops.  Returns (ms_per_layer, cores, sample_text)."""
     from oracle import ref
@@ -131,21 +139,21 @@ def oracle_sample_ms_per_layer(cfg, budget_s=12.0):
     # calibrate with a small probe, then size the sample for ~budget_s
     def run_feature(rows):
         t = time.perf_counter()
-        ref.feature_fwd(feat["Q"], feat["K"], feat["V"], cv_s, rows=rows)
-        ref.feature_bwd(feat["Q"], feat["K"], feat["V"], feat["dO"], cv_s, rows=rows)
+        ref.feature_fwd(feat["Q"], feat["K"], feat["V"], cv_s, rows=rows, nthreads=nthreads)
+        ref.feature_bwd(feat["Q"], feat["K"], feat["V"], feat["dO"], cv_s, rows=rows, nthreads=nthreads)
         fl = sum(14 * int(cvn[b]) ** 2 * sub.d for b, _ in rows)
         return time.perf_counter() - t, fl
 
     def run_item(cols):
         t = time.perf_counter()
-        ref.item_fwd(item["Q"], item["K"], item["V"], nt_s, cv_s, cols=cols)
-        ref.item_bwd(item["Q"], item["K"], item["V"], item["dO"], nt_s, cv_s, cols=cols)
+        ref.item_fwd(item["Q"], item["K"], item["V"], nt_s, cv_s, cols=cols, nthreads=nthreads)
+        ref.item_bwd(item["Q"], item["K"], item["V"], item["dO"], nt_s, cv_s, cols=cols, nthreads=nthreads)
         fl = sum(14 * sub.R * int(nt_s[b]) * sub.d for b, _ in cols)
         return time.perf_counter() - t, fl
 
     valid_cols = [(b, c) for b in range(sub.B) for c in range(sub.C) if cv_s is None or cv_s[b, c]]
     all_rows = [(b, r) for b in range(sub.B) for r in range(sub.R)]
-    threads = ref.num_threads()
+    threads = nthreads if nthreads > 0 else ref.num_threads()
     probe_c = [valid_cols[i] for i in rng.choice(len(valid_cols), size=min(threads, len(valid_cols)), replace=False)]
     tc, fc = run_item(probe_c)
     n_cols = int(max(threads, min(len(valid_cols), (0.7 * budget_s / max(tc, 1e-6)) * len(probe_c))))
@@ -213,6 +221,161 @@ def job_value(ms_per_step, layers, world):
 
 
 # ---- our arm ----------------------------------------------------------------------------------------
+CALLS = ("feature_fwd", "item_fwd", "item_bwd", "feature_bwd")
+
+
+def pick_tensor_peak(peaks, region_s):
+    """Guide rule (B200_PROFILING.md): the burst bf16 figure for a kernel timed alone, the sustained one for
+    a kernel timed inside a long step.  A timed region of >= 1 s is 'long'."""
+    if region_s >= 1.0:
+        return peaks["bf16_tflops_sustained"], "sustained"
+    return peaks["bf16_tflops"], "burst"
+
+
+def call_table(call_ms, work, peaks, region_s):
+    tpeak, tkind = pick_tensor_peak(peaks, region_s)
+    out = {}
+    for n in CALLS:
+        ms = call_ms[n]
+        tf = work[n + "_flops"] / (ms * 1e-3) / 1e12
+        gb = work[n + "_bytes"] / (ms * 1e-3) / 1e9
+        out[n] = {"ms": ms, "TFLOP/s": tf, "GB/s": gb,
+                  "frac_tensor": tf / tpeak, "frac_tensor_kind": tkind,
+                  "frac_tensor_sustained": tf / peaks["bf16_tflops_sustained"],
+                  "frac_tensor_burst": tf / peaks["bf16_tflops"],
+                  "frac_tensor_nominal": tf / NOMINAL_PEAKS["bf16_tflops"],
+                  "frac_hbm": gb / peaks["hbm_gbs"], "frac_hbm_nominal": gb / NOMINAL_PEAKS["hbm_gbs"]}
+    return out
+
+
+class Workload:
+    """One config resident in HBM: per-layer inputs, per-layer forward outputs (the backward of layer l
+    reads its own O/LSE, reading c17), shared gradient buffers and workspace."""
+
+    def __init__(self, torch, tab, cfg, dev):
+        self.torch, self.tab, self.cfg = torch, tab, cfg
+        self.n_train_h, self.col_valid_h = draw_structure(cfg)
+        self.n_train = torch.from_numpy(self.n_train_h).to(dev)
+        self.col_valid = torch.from_numpy(self.col_valid_h).to(dev) if self.col_valid_h is not None else None
+        self.work = algorithmic_work(cfg, self.n_train_h, self.col_valid_h)
+        x_cache = {}
+        self.layers = [{ax: make_call_inputs(cfg, ax, l, device=dev, x_cache=x_cache) for ax in ("feature", "item")}
+                       for l in range(cfg.layers)]
+        x_cache.clear()
+        shp = (cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh)
+        bf = dict(dtype=torch.bfloat16, device=dev)
+        f32 = dict(dtype=torch.float32, device=dev)
+        self.fwd = [{"O_f": torch.empty(shp, **bf), "O_i": torch.empty(shp, **bf),
+                     "LSE_f": torch.empty((cfg.B, cfg.R, cfg.H, cfg.C), **f32),
+                     "LSE_i": torch.empty((cfg.B, cfg.C, cfg.H, cfg.R), **f32)} for _ in range(cfg.layers)]
+        self.buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)   # gradients + workspace
+        self.stream = torch.cuda.current_stream()
+        self.reps = 1
+
+    @property
+    def calls_per_step(self):
+        return 4 * self.cfg.layers * self.reps
+
+    def names_in_order(self):
+        one = ["feature_fwd", "item_fwd"] * self.cfg.layers + ["item_bwd", "feature_bwd"] * self.cfg.layers
+        return one * self.reps
+
+    def step(self, events=None):
+        tab, buf, nt, cv, nth = self.tab, self.buf, self.n_train, self.col_valid, self.n_train_h
+        i = 0
+
+        def rec():
+            nonlocal i
+            if events is not None:
+                events[i].record(self.stream)
+                i += 1
+        rec()
+        for _ in range(self.reps):
+            for L, F in zip(self.layers, self.fwd):
+                f, it = L["feature"], L["item"]
+                tab.tabattn_feature_fwd(f["Q"], f["K"], f["V"], cv, O=F["O_f"], LSE=F["LSE_f"], ws=buf.ws)
+                rec()
+                tab.tabattn_item_fwd(it["Q"], it["K"], it["V"], nt, cv, n_train_host=nth, O=F["O_i"],
+                                     LSE=F["LSE_i"], ws=buf.ws)
+                rec()
+            for L, F in zip(reversed(self.layers), reversed(self.fwd)):
+                f, it = L["feature"], L["item"]
+                tab.tabattn_item_bwd(it["Q"], it["K"], it["V"], F["O_i"], it["dO"], F["LSE_i"], nt, cv,
+                                     n_train_host=nth, dQ=buf.grads_i[0], dK=buf.grads_i[1], dV=buf.grads_i[2],
+                                     ws=buf.ws)
+                rec()
+                tab.tabattn_feature_bwd(f["Q"], f["K"], f["V"], F["O_f"], f["dO"], F["LSE_f"], cv,
+                                        dQ=buf.grads_f[0], dK=buf.grads_f[1], dV=buf.grads_f[2], ws=buf.ws)
+                rec()
+
+
+def time_workload(torch, dist, tab, wl, steps, warmup, min_region_s, world, rank, local, dev):
+    """W warm-up steps, then exactly K timed steps bracketed by barrier + synchronize; device time from
+    CUDA events on the launching stream, max over ranks.  Returns the measurement dict."""
+    cfg = wl.cfg
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # calibration (untimed): size the step so that K steps last >= min_region_s
+    wl.reps = 1
+    wl.step()
+    barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(wl.stream)
+    wl.step()
+    b.record(wl.stream)
+    barrier()
+    est = max_over_ranks(a.elapsed_time(b), world, dev)
+    wl.reps = int(max(1, min(256, -(-min_region_s * 1e3 // max(steps * est, 1e-3)))))
+    for _ in range(warmup):
+        wl.step()
+    barrier()
+    n_ev = wl.calls_per_step + 1
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(n_ev)] for _ in range(steps)]
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    launches0 = tab.launch_count()
+    t0.record(wl.stream)
+    for k in range(steps):
+        wl.step(ev[k])
+    t1.record(wl.stream)
+    barrier()
+    launches = tab.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks(t0.elapsed_time(t1), world, dev)
+    names = wl.names_in_order()
+    acc = {n: [] for n in CALLS}
+    for k in range(steps):
+        for i, n in enumerate(names):
+            acc[n].append(ev[k][i].elapsed_time(ev[k][i + 1]))
+    call_ms = {n: float(np.mean(v)) for n, v in acc.items()}
+    layers_per_step = cfg.layers * wl.reps
+    return {"total_ms": total_ms, "ms_per_step": total_ms / steps, "layers_per_step": layers_per_step,
+            "ms_per_layer": total_ms / steps / layers_per_step, "region_s": total_ms * 1e-3,
+            "call_ms": call_ms, "launches": int(launches), "clocks": clocks}
+
+
+def static_traffic(cfg_name, call):
+    """DRAM bytes (read + write) of one C-ABI call from the committed ncu --set full capture
+    (profiles/r02_traffic.csv; falls back to round 1's).  A static capture, not measured in this run."""
+    for fn in ("r02_traffic.csv", "r01_traffic.csv"):
+        path = os.path.join(ROOT, "profiles", fn)
+        if not os.path.exists(path):
+            continue
+        for row in open(path).read().splitlines()[1:]:
+            f = row.split(",")
+            if len(f) >= 3 and f[0] == cfg_name and f[1] == call:
+                return int(f[2]), "profiles/" + fn + " (static ncu --set full capture, per call)"
+    return None, None
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -227,81 +390,24 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-    cfg = get_config(args.config)
-    n_train_h, col_valid_h = draw_structure(cfg)
-    n_train = torch.from_numpy(n_train_h).to(dev)
-    col_valid = torch.from_numpy(col_valid_h).to(dev) if col_valid_h is not None else None
-    work = algorithmic_work(cfg, n_train_h, col_valid_h)
-
-    # inputs: resident in HBM before the timed region.  Every layer has its own Q,K,V,dO per axis
-    # (replicas only across ranks: each rank runs the same seeded workload on its own GPU).
-    x_cache = {}
-    layers = []
-    for l in range(cfg.layers):
-        layers.append({ax: make_call_inputs(cfg, ax, l, device=dev, x_cache=x_cache) for ax in ("feature", "item")})
-    x_cache.clear()
-    buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
-    stream = torch.cuda.current_stream()
-
-    def step(events=None):
-        # forward calls in layer order, then backward calls in reverse order would need per-layer O/LSE
-        # buffers; per layer the four calls run back to back (reading c17: chained = enqueued back to back)
-        for li, L in enumerate(layers):
-            f, it = L["feature"], L["item"]
-            if events is not None:
-                events[li][0].record(stream)
-            tab.tabattn_feature_fwd(f["Q"], f["K"], f["V"], col_valid, O=buf.O_f, LSE=buf.LSE_f, ws=buf.ws)
-            if events is not None:
-                events[li][1].record(stream)
-            tab.tabattn_item_fwd(it["Q"], it["K"], it["V"], n_train, col_valid, n_train_host=n_train_h,
-                                 O=buf.O_i, LSE=buf.LSE_i, ws=buf.ws)
-            if events is not None:
-                events[li][2].record(stream)
-            tab.tabattn_item_bwd(it["Q"], it["K"], it["V"], buf.O_i, it["dO"], buf.LSE_i, n_train, col_valid,
-                                 n_train_host=n_train_h, dQ=buf.grads_i[0], dK=buf.grads_i[1], dV=buf.grads_i[2],
-                                 ws=buf.ws)
-            if events is not None:
-                events[li][3].record(stream)
-            tab.tabattn_feature_bwd(f["Q"], f["K"], f["V"], buf.O_f, f["dO"], buf.LSE_f, col_valid,
-                                    dQ=buf.grads_f[0], dK=buf.grads_f[1], dV=buf.grads_f[2], ws=buf.ws)
-            if events is not None:
-                events[li][4].record(stream)
+    peaks = load_peaks()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    ev = [[[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in layers] for _ in range(args.steps)]
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-        time.sleep(0.12)
-    barrier()
-    launches0 = tab.launch_count()
-    t0.record(stream)
-    for k in range(args.steps):
-        step(ev[k])
-    t1.record(stream)
-    barrier()
-    launches = tab.launch_count() - launches0
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = max_over_ranks(t0.elapsed_time(t1), world, dev)
-    ms_per_step = total_ms / args.steps
-    # per-call device times (mean over steps and layers), from events on the launching stream
-    names = ["feature_fwd", "item_fwd", "item_bwd", "feature_bwd"]
-    call_ms = {n: float(np.mean([ev[k][li][i].elapsed_time(ev[k][li][i + 1])
-                                 for k in range(args.steps) for li in range(len(layers))]))
-               for i, n in enumerate(names)}
+    # ---- headline config: inputs resident in HBM before the timed region (replicas only across ranks:
+    # each rank runs the same seeded workload on its own GPU)
+    cfg = get_config(args.config)
+    wl = Workload(torch, tab, cfg, dev)
+    m = time_workload(torch, dist, tab, wl, args.steps, args.warmup, args.min_region, world, rank, local, dev)
+    work, call_ms = wl.work, m["call_ms"]
 
     # ---- end to end from pinned host buffers (layer 0), H2D + 4 calls + D2H every step ----------------
     e2e = None
     if not args.no_e2e:
-        L0 = layers[0]
+        L0 = wl.layers[0]
         host = {ax: {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in L0[ax].items()}
                 for ax in ("feature", "item")}
         stage = {ax: {k: torch.empty_like(v) for k, v in L0[ax].items()} for ax in ("feature", "item")}
@@ -309,72 +415,93 @@ def run_ours(args):
         e_steps = max(1, min(args.steps, 5))
         for _ in range(2):
             h2d, d2h = tab.layer_fwd_bwd_host(host["feature"], host["item"], stage["feature"], stage["item"],
-                                              out_host, n_train, col_valid, buf, n_train_h)
+                                              out_host, wl.n_train, wl.col_valid, wl.buf, wl.n_train_h)
         barrier()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
+        a.record(wl.stream)
         for _ in range(e_steps):
             h2d, d2h = tab.layer_fwd_bwd_host(host["feature"], host["item"], stage["feature"], stage["item"],
-                                              out_host, n_train, col_valid, buf, n_train_h)
-        b.record(stream)
+                                              out_host, wl.n_train, wl.col_valid, wl.buf, wl.n_train_h)
+        b.record(wl.stream)
         barrier()
         et = max_over_ranks(a.elapsed_time(b) / e_steps, world, dev)
         e2e = {"value": job_value(et, 1, world), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "note": "one layer per step from pinned host buffers, pipelined over up to 16 table groups (H2D, kernels, D2H on three streams)"}
+               "d2h_bytes_per_step": int(d2h), "steps": e_steps,
+               "note": "one layer per step through layer_fwd_bwd_host (the public API) from pinned host buffers, "
+                       "pipelined over up to 16 table groups (H2D, kernels, D2H on three streams); PCIe-bound"}
         del host, stage, out_host
+    n_train_h, col_valid_h = wl.n_train_h, wl.col_valid_h
+    del wl
+    torch.cuda.empty_cache()
+
+    # ---- the other timed configs, same protocol, same run (single GPU only) ----------------------------
+    others = {}
+    if world == 1 and not args.no_extra:
+        for name in SECONDARY:
+            if name == cfg.name:
+                continue
+            c2 = get_config(name)
+            w2 = Workload(torch, tab, c2, dev)
+            m2 = time_workload(torch, dist, tab, w2, args.steps, args.warmup, args.min_region, world, rank, local, dev)
+            others[name] = {"ms_per_layer": m2["ms_per_layer"], "ms_per_step": m2["ms_per_step"], "steps": args.steps,
+                            "layers_per_step": m2["layers_per_step"], "timed_region_s": m2["region_s"],
+                            "gpu_launches": m2["launches"], "clocks": m2["clocks"],
+                            "calls": call_table(m2["call_ms"], w2.work, peaks, m2["region_s"])}
+            del w2
+            torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    peaks = load_peaks()
-    # dominant call of the step and its roofline
+    # ---- roofline of the dominant call of the headline step -----------
     dom = max(call_ms, key=call_ms.get)
+    region_s = m["region_s"]
     if dom.startswith("item"):
         flops = work[dom + "_flops"]
         ach = flops / (call_ms[dom] * 1e-3) / 1e12
-        peak = peaks["bf16_tflops_sustained"]
+        peak, kind = pick_tensor_peak(peaks, region_s)
         roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": None, "kernel": "tabattn_" + dom, "peak_source": peaks["source"] + " (sustained bf16)",
-                "algorithmic_flops_per_launch": flops}
+                "peak_kind": "%s bf16 %s (timed region %.2f s)" % (peaks["source"], kind, region_s),
+                "frac_vs": {"measured_sustained": ach / peaks["bf16_tflops_sustained"],
+                            "measured_burst": ach / peaks["bf16_tflops"],
+                            "nominal_2.25PF": ach / NOMINAL_PEAKS["bf16_tflops"]},
+                "kernel": "tabattn_" + dom, "algorithmic_flops_per_launch": flops}
     else:
         nbytes = work[dom + "_bytes"]
         ach = nbytes / (call_ms[dom] * 1e-3) / 1e9
         peak = peaks["hbm_gbs"]
         roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "kernel": "tabattn_" + dom, "peak_source": peaks["source"],
-                "algorithmic_bytes_per_launch": nbytes}
-    traffic_file = os.path.join(ROOT, "profiles", "r01_traffic.csv")   # ncu --set full DRAM bytes per call
-    if os.path.exists(traffic_file):
-        for row in open(traffic_file).read().splitlines()[1:]:
-            f = row.split(",")
-            if len(f) == 3 and f[0] == cfg.name and f[1] == dom:
-                roof["traffic"] = int(f[2])
-    calls = {}
-    for n in names:
-        ms = call_ms[n]
-        calls[n] = {"ms": ms, "TFLOP/s": work[n + "_flops"] / (ms * 1e-3) / 1e12,
-                    "GB/s": work[n + "_bytes"] / (ms * 1e-3) / 1e9,
-                    "frac_tensor": work[n + "_flops"] / (ms * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
-                    "frac_hbm": work[n + "_bytes"] / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+                "peak_kind": "%s copy bandwidth" % peaks["source"],
+                "frac_vs": {"measured_copy": ach / peak, "nominal_8TBs": ach / NOMINAL_PEAKS["hbm_gbs"]},
+                "kernel": "tabattn_" + dom, "algorithmic_bytes_per_launch": nbytes}
+    roof["traffic"], roof["traffic_source"] = static_traffic(cfg.name, dom)
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         ms_cpu, cores, sample, _ = oracle_sample_ms_per_layer(cfg, budget_s=args.cpu_budget)
         cpu = {"value": ms_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        ms_1, _, sample_1, _ = oracle_sample_ms_per_layer(cfg, budget_s=args.cpu_budget, nthreads=1)
+        cpu["one_core"] = {"value": ms_1, "unit": UNIT, "cores": 1, "sample": sample_1}
 
-    value = job_value(ms_per_step, cfg.layers, world)
+    value = job_value(m["ms_per_step"], m["layers_per_step"], world)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": m["ms_per_step"], "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": cfg.name, "B": cfg.B, "R": cfg.R, "C": cfg.C, "H": cfg.H, "dh": cfg.dh,
-                       "layers": cfg.layers, "n_train": [int(n_train_h.min()), int(n_train_h.max())],
+                       "layers": cfg.layers, "layers_per_step": m["layers_per_step"],
+                       "timed_region_s": region_s,
+                       "n_train": [int(n_train_h.min()), int(n_train_h.max())],
                        "masked": col_valid_h is not None, "parallelism": "replicas x%d" % world,
-                       "l2": "inputs larger than L2 (%.0f MB read per step); no flush"
+                       "order": "forward calls of all layers of the step in layer order, then backward calls in "
+                                "reverse (reading c17); the step repeats the config's layers until K steps last "
+                                ">= %.1f s" % args.min_region,
+                       "l2": "inputs larger than L2 (%.0f MB read per layer); no flush"
                              % ((work["feature_fwd_bytes"] + work["item_fwd_bytes"]) / 1e6)},
-            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-            "clocks": clocks, "calls": calls,
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
+            "clocks": m["clocks"], "calls": call_table(call_ms, work, peaks, region_s), "configs": others,
+            "peaks": {k: peaks[k] for k in ("hbm_gbs", "bf16_tflops", "bf16_tflops_sustained", "source")},
             "context": {"paper_l40s_baseline_min": 74.32, "paper_l40s_record_min": 0.92,
                         "note": "full-pretraining wallclock on 1x L40S (PAPER.md:L43, L51); context, not the target"}}
     print(json.dumps(line))
@@ -388,11 +515,13 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="base")
+    ap.add_argument("--config", default="long_item")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--min-region", type=float, default=3.0, help="seconds the K timed steps must last at least")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-budget", type=float, default=12.0)
+    ap.add_argument("--no-extra", action="store_true", help="skip the secondary configs")
+    ap.add_argument("--cpu-budget", type=float, default=10.0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -13,7 +13,10 @@
  * _host.  The caller owns every buffer; the library allocates no device memory,
  * never synchronises the host, and enqueues all work on `stream` (graph-capturable).
  * Outputs are fully overwritten; inputs are never written; no aliasing of an output
- * with any other argument.
+ * with any other argument.  Calls are re-entrant across host threads and across devices
+ * (the device is the calling thread's current CUDA device; it must be sm_100): the only
+ * process-wide state is a mutex-protected cache of TMA descriptors and per-device launch
+ * attributes.  Concurrent calls must use different workspaces.
  *
  * Feature attention (a1/a2 of SURVEY.md §8(a)): for each (b, r, h) the sequence runs
  *   over the table's VALID columns:  S = scale * Q K^T (Cv x Cv), P = softmax_rows(S),
@@ -49,9 +52,11 @@ extern "C" {
 typedef enum {
   TABATTN_OK = 0,
   TABATTN_ERR_INVALID_ARG = 1, /* NULL required pointer, non-positive size, misaligned pointer,
-                                  n_train_host[b] outside [1,R], NULL shape */
+                                  n_train_host[b] outside [1,R], NULL shape, an output pointer equal
+                                  to another argument's pointer (aliasing) */
   TABATTN_ERR_UNSUPPORTED = 2, /* dh not in {16,32,64}, C > TABATTN_MAX_FEATURE_C for feature_*,
-                                  tensor larger than 2^31 cells, device is not sm_100 */
+                                  H*dh > TABATTN_MAX_D, B*R*C >= 2^31 cells, the calling thread's
+                                  current device is not sm_100 */
   TABATTN_ERR_WORKSPACE = 3,   /* ws == NULL or ws_bytes < tabattn_workspace_bytes(shape, op) */
   TABATTN_ERR_CUDA = 4         /* a CUDA launch / driver call failed (see cudaGetLastError) */
 } tabattn_status;
@@ -60,6 +65,7 @@ typedef enum {
 enum { TABATTN_OP_FEATURE_FWD = 0, TABATTN_OP_FEATURE_BWD = 1, TABATTN_OP_ITEM_FWD = 2, TABATTN_OP_ITEM_BWD = 3 };
 
 #define TABATTN_MAX_FEATURE_C 128 /* largest column count the feature kernels accept */
+#define TABATTN_MAX_D 4096        /* largest embedding width d = H*dh any call accepts  */
 
 typedef struct {
   int32_t B, R, C, H, dh;       /* all >= 1; dh in {16, 32, 64}                                    */
@@ -90,8 +96,9 @@ TABATTN_API tabattn_status tabattn_feature_bwd(const tabattn_shape* shape, const
 TABATTN_API tabattn_status tabattn_item_fwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
                                 void* O, float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream);
 
-/* Item attention backward: a dQ pass (also emits D = rowsum(dO o O) into the workspace) and a
- * separate dK/dV pass; deterministic, no atomics. */
+/* Item attention backward: a dQ pass (it also computes D = rowsum(dO o O) and -LSE*log2(e) per query
+ * row and leaves them in the workspace) and a separate dK/dV pass that reads them; two kernel
+ * launches, deterministic, no atomics.  ws: tabattn_workspace_bytes(shape, TABATTN_OP_ITEM_BWD). */
 TABATTN_API tabattn_status tabattn_item_bwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
                                 const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
                                 void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);

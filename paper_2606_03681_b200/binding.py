@@ -9,6 +9,7 @@ Tensors are ``[B,R,C,H,dh]`` torch.bfloat16 CUDA tensors, contiguous; ``n_train`
 CUDA tensor ``[B]``; ``col_valid`` an optional uint8 CUDA tensor ``[B,C]``.  Feature LSE is
 ``[B,R,H,C]`` f32, item LSE ``[B,C,H,R]`` f32.
 """
+import contextlib
 import ctypes
 import os
 
@@ -107,24 +108,55 @@ def workspace_bytes(shape: TabattnShape, op: int) -> int:
 
 
 def _check_inputs(*ts):
+    """Cell tensors (inputs and caller-provided outputs): contiguous CUDA bfloat16 [B,R,C,H,dh] on one device."""
     t0 = ts[0]
-    for t in ts:
-        if t.dtype != torch.bfloat16 or not t.is_cuda or not t.is_contiguous() or t.shape != t0.shape:
-            raise ValueError("tensors must be contiguous CUDA bfloat16 of one shape [B,R,C,H,dh]")
     if t0.dim() != 5:
         raise ValueError("expected [B,R,C,H,dh]")
+    for t in ts:
+        if t is None:
+            continue
+        if (t.dtype != torch.bfloat16 or not t.is_cuda or not t.is_contiguous() or t.shape != t0.shape
+                or t.device != t0.device):
+            raise ValueError("tensors must be contiguous CUDA bfloat16 of one shape [B,R,C,H,dh] on one device")
 
 
-def _stream(stream):
+def _check_aux(Q, n_train=None, col_valid=None, LSE=None, lse_shape=None):
+    """The non-cell arguments cross the ABI as raw pointers: a wrong dtype would be read as garbage
+    (torch's default int64 n_train reads as int32 pairs), so it is rejected here."""
+    B, R, C, H, dh = Q.shape
+    if n_train is not None:
+        if (n_train.dtype != torch.int32 or not n_train.is_cuda or not n_train.is_contiguous()
+                or tuple(n_train.shape) != (B,) or n_train.device != Q.device):
+            raise ValueError("n_train must be a contiguous CUDA int32 tensor [B] on the device of Q")
+    if col_valid is not None:
+        if (col_valid.dtype not in (torch.uint8, torch.bool) or not col_valid.is_cuda
+                or not col_valid.is_contiguous() or tuple(col_valid.shape) != (B, C) or col_valid.device != Q.device):
+            raise ValueError("col_valid must be a contiguous CUDA uint8/bool tensor [B,C] on the device of Q")
+    if LSE is not None:
+        if (LSE.dtype != torch.float32 or not LSE.is_cuda or not LSE.is_contiguous()
+                or tuple(LSE.shape) != tuple(lse_shape) or LSE.device != Q.device):
+            raise ValueError("LSE must be a contiguous CUDA float32 tensor %s on the device of Q" % (lse_shape,))
+
+
+def _on(device):
+    """Make `device` the calling thread's current CUDA device for the ABI call (the library launches on it)."""
+    if device.index is None or device.index == torch.cuda.current_device():
+        return contextlib.nullcontext()
+    return torch.cuda.device(device)
+
+
+def _stream(stream, device):
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(device)
     return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
 
 
-def _workspace(shape, op, ws):
+def _workspace(shape, op, ws, device):
     need = workspace_bytes(shape, op)
     if ws is None and need:
-        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        ws = torch.empty(need, dtype=torch.uint8, device=device)
+    if ws is not None and (not ws.is_cuda or not ws.is_contiguous() or ws.device != device):
+        raise ValueError("ws must be a contiguous CUDA tensor on the device of Q")
     return ws, (ws.numel() * ws.element_size() if ws is not None else 0)
 
 
@@ -135,14 +167,16 @@ def _raise(st, what):
 
 def tabattn_feature_fwd(Q, K, V, col_valid=None, softmax_scale=0.0, O=None, LSE=None, ws=None, stream=None):
     """Feature-axis attention forward (tabattn.h: tabattn_feature_fwd).  Returns (O, LSE[B,R,H,C])."""
-    _check_inputs(Q, K, V)
+    _check_inputs(Q, K, V, O)
     B, R, C, H, dh = Q.shape
+    _check_aux(Q, None, col_valid, LSE, (B, R, H, C))
     shape, keep = make_shape(Q, None, col_valid, None, softmax_scale)
     O = torch.empty_like(Q) if O is None else O
     LSE = torch.empty((B, R, H, C), dtype=torch.float32, device=Q.device) if LSE is None else LSE
-    ws, nws = _workspace(shape, OP_FEATURE_FWD, ws)
-    st = lib().tabattn_feature_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
-                                   _ptr(ws), nws, _stream(stream))
+    ws, nws = _workspace(shape, OP_FEATURE_FWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_feature_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
+                                       _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_feature_fwd")
     return O, LSE
 
@@ -150,14 +184,18 @@ def tabattn_feature_fwd(Q, K, V, col_valid=None, softmax_scale=0.0, O=None, LSE=
 def tabattn_feature_bwd(Q, K, V, O, dO, LSE, col_valid=None, softmax_scale=0.0, dQ=None, dK=None, dV=None,
                         ws=None, stream=None):
     """Feature-axis attention backward (tabattn.h: tabattn_feature_bwd).  Returns (dQ, dK, dV)."""
-    _check_inputs(Q, K, V, O, dO)
+    _check_inputs(Q, K, V, O, dO, dQ, dK, dV)
+    B, R, C, H, dh = Q.shape
+    _check_aux(Q, None, col_valid, LSE, (B, R, H, C))
     shape, keep = make_shape(Q, None, col_valid, None, softmax_scale)
     dQ = torch.empty_like(Q) if dQ is None else dQ
     dK = torch.empty_like(Q) if dK is None else dK
     dV = torch.empty_like(Q) if dV is None else dV
-    ws, nws = _workspace(shape, OP_FEATURE_BWD, ws)
-    st = lib().tabattn_feature_bwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(LSE),
-                                   _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), nws, _stream(stream))
+    ws, nws = _workspace(shape, OP_FEATURE_BWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_feature_bwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO),
+                                       _ptr(LSE), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), nws,
+                                       _stream(stream, Q.device))
     _raise(st, "tabattn_feature_bwd")
     return dQ, dK, dV
 
@@ -165,14 +203,16 @@ def tabattn_feature_bwd(Q, K, V, O, dO, LSE, col_valid=None, softmax_scale=0.0, 
 def tabattn_item_fwd(Q, K, V, n_train, col_valid=None, softmax_scale=0.0, n_train_host=None, O=None, LSE=None,
                      ws=None, stream=None):
     """Item-axis attention forward (tabattn.h: tabattn_item_fwd).  Returns (O, LSE[B,C,H,R])."""
-    _check_inputs(Q, K, V)
+    _check_inputs(Q, K, V, O)
     B, R, C, H, dh = Q.shape
+    _check_aux(Q, n_train, col_valid, LSE, (B, C, H, R))
     shape, keep = make_shape(Q, n_train, col_valid, n_train_host, softmax_scale)
     O = torch.empty_like(Q) if O is None else O
     LSE = torch.empty((B, C, H, R), dtype=torch.float32, device=Q.device) if LSE is None else LSE
-    ws, nws = _workspace(shape, OP_ITEM_FWD, ws)
-    st = lib().tabattn_item_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
-                                _ptr(ws), nws, _stream(stream))
+    ws, nws = _workspace(shape, OP_ITEM_FWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_item_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
+                                    _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_item_fwd")
     return O, LSE
 
@@ -180,13 +220,16 @@ def tabattn_item_fwd(Q, K, V, n_train, col_valid=None, softmax_scale=0.0, n_trai
 def tabattn_item_bwd(Q, K, V, O, dO, LSE, n_train, col_valid=None, softmax_scale=0.0, n_train_host=None,
                      dQ=None, dK=None, dV=None, ws=None, stream=None):
     """Item-axis attention backward (tabattn.h: tabattn_item_bwd).  Returns (dQ, dK, dV)."""
-    _check_inputs(Q, K, V, O, dO)
+    _check_inputs(Q, K, V, O, dO, dQ, dK, dV)
+    B, R, C, H, dh = Q.shape
+    _check_aux(Q, n_train, col_valid, LSE, (B, C, H, R))
     shape, keep = make_shape(Q, n_train, col_valid, n_train_host, softmax_scale)
     dQ = torch.empty_like(Q) if dQ is None else dQ
     dK = torch.empty_like(Q) if dK is None else dK
     dV = torch.empty_like(Q) if dV is None else dV
-    ws, nws = _workspace(shape, OP_ITEM_BWD, ws)
-    st = lib().tabattn_item_bwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(LSE),
-                                _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), nws, _stream(stream))
+    ws, nws = _workspace(shape, OP_ITEM_BWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_item_bwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(LSE),
+                                    _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_item_bwd")
     return dQ, dK, dV

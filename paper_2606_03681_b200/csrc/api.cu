@@ -26,8 +26,7 @@ tabattn_status check_shape(const tabattn_shape* sh, bool item, Shape* out) {
   if (sh->B < 1 || sh->R < 1 || sh->C < 1 || sh->H < 1 || sh->dh < 1) return TABATTN_ERR_INVALID_ARG;
   if (sh->dh != 16 && sh->dh != 32 && sh->dh != 64) return TABATTN_ERR_UNSUPPORTED;
   const long long cells = (long long)sh->B * sh->R * sh->C;
-  if (cells >= (1LL << 31) || (long long)sh->B * sh->C > 65535 || (long long)sh->H * sh->dh > 4096)
-    return TABATTN_ERR_UNSUPPORTED;
+  if (cells >= (1LL << 31) || (long long)sh->H * sh->dh > TABATTN_MAX_D) return TABATTN_ERR_UNSUPPORTED;
   if (item) {
     if (!sh->n_train) return TABATTN_ERR_INVALID_ARG;
     if (sh->n_train_host)
@@ -42,16 +41,24 @@ tabattn_status check_shape(const tabattn_shape* sh, bool item, Shape* out) {
   return TABATTN_OK;
 }
 
+// The calling thread's current device must be sm_100 (per-device, thread-safe: device.cu).
 tabattn_status check_device() {
-  static int cached = -1;  // 1 = sm_100, 0 = other
-  if (cached < 0) {
-    int dev = 0, major = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return TABATTN_ERR_CUDA;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
-      return TABATTN_ERR_CUDA;
-    cached = (major == 10) ? 1 : 0;
+  const tabattn::DeviceInfo* di = tabattn::current_device();
+  if (!di) return TABATTN_ERR_CUDA;
+  return di->cc_major == 10 ? TABATTN_OK : TABATTN_ERR_UNSUPPORTED;
+}
+
+// Outputs may not alias any other argument (tabattn.h): equal base pointers are rejected.  (Partial
+// overlaps of distinct allocations cannot be told from here and stay the caller's responsibility.)
+template <size_t NO, size_t NI>
+bool aliased(const void* const (&outs)[NO], const void* const (&ins)[NI]) {
+  for (size_t i = 0; i < NO; ++i) {
+    for (size_t j = i + 1; j < NO; ++j)
+      if (outs[i] == outs[j]) return true;
+    for (size_t j = 0; j < NI; ++j)
+      if (outs[i] == ins[j]) return true;
   }
-  return cached == 1 ? TABATTN_OK : TABATTN_ERR_UNSUPPORTED;
+  return false;
 }
 
 template <typename... P>
@@ -98,7 +105,6 @@ size_t tabattn_workspace_bytes(const tabattn_shape* sh, int op) {
   tmp.n_train_host = nullptr;
   if (check_shape(&tmp, op >= 2, &s) != TABATTN_OK) return 0;
   switch (op) {
-    case TABATTN_OP_ITEM_FWD: return tabattn::item_fwd_workspace_bytes(s);
     case TABATTN_OP_ITEM_BWD: return tabattn::item_bwd_workspace_bytes(s);
     default: return 0;
   }
@@ -111,6 +117,11 @@ tabattn_status tabattn_feature_fwd(const tabattn_shape* sh, const void* Q, const
   tabattn_status st = check_shape(sh, false, &s);
   if (st != TABATTN_OK) return st;
   if (!all_ok(Q, K, V, (const void*)O, (const void*)LSE)) return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {O, LSE};
+    const void* const ins[] = {Q, K, V};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
   if ((st = check_device()) != TABATTN_OK) return st;
   return from_cuda(tabattn::launch_feature_fwd(s, Q, K, V, O, LSE, (cudaStream_t)stream));
 }
@@ -124,6 +135,11 @@ tabattn_status tabattn_feature_bwd(const tabattn_shape* sh, const void* Q, const
   if (st != TABATTN_OK) return st;
   if (!all_ok(Q, K, V, O, dO, (const void*)LSE, (const void*)dQ, (const void*)dK, (const void*)dV))
     return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {dQ, dK, dV};
+    const void* const ins[] = {Q, K, V, O, dO, LSE};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
   if ((st = check_device()) != TABATTN_OK) return st;
   return from_cuda(tabattn::launch_feature_bwd(s, Q, K, V, O, dO, LSE, dQ, dK, dV, (cudaStream_t)stream));
 }
@@ -133,10 +149,15 @@ tabattn_status tabattn_item_fwd(const tabattn_shape* sh, const void* Q, const vo
   Shape s;
   tabattn_status st = check_shape(sh, true, &s);
   if (st != TABATTN_OK) return st;
+  (void)ws; (void)ws_bytes;
   if (!all_ok(Q, K, V, (const void*)O, (const void*)LSE)) return TABATTN_ERR_INVALID_ARG;
-  if ((st = check_ws(tabattn::item_fwd_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
+  {
+    const void* const outs[] = {O, LSE};
+    const void* const ins[] = {Q, K, V};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, ws, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_item_bwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V,
@@ -147,9 +168,15 @@ tabattn_status tabattn_item_bwd(const tabattn_shape* sh, const void* Q, const vo
   if (st != TABATTN_OK) return st;
   if (!all_ok(Q, K, V, O, dO, (const void*)LSE, (const void*)dQ, (const void*)dK, (const void*)dV))
     return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {dQ, dK, dV, ws};
+    const void* const ins[] = {Q, K, V, O, dO, LSE};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
   if ((st = check_ws(tabattn::item_bwd_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_item_bwd(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_item_bwd(s, Q, K, V, O, dO, LSE, dQ, dK, dV, static_cast<float*>(ws),
+                                            (cudaStream_t)stream));
 }
 
 }  // extern "C"

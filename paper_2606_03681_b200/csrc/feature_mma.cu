@@ -964,7 +964,7 @@ cudaError_t launch_persistent(Kern kern, const Plan& pl, cudaStream_t stream, Ar
   if (e != cudaSuccess) return e;
   if (occ < 1) return cudaErrorInvalidValue;
   const int per_sm = occ < pl.ctas_per_sm ? occ : pl.ctas_per_sm;
-  const long long want = (long long)num_sms() * per_sm;
+  const long long want = (long long)current_device()->num_sms * per_sm;
   const int grid = (int)(pl.p.n_su < want ? pl.p.n_su : want);
   if (env_int("TABATTN_FEAT_DEBUG", 0))
     fprintf(stderr, "feature plan: hg=%d rows=%d warps=%d nstage=%d stage=%u B smem=%zu B occ=%d ctas/sm=%d grid=%d\n",

@@ -1,6 +1,6 @@
-// Item-axis attention backward on tcgen05: a small prep kernel
-// (D = rowsum(dO o O) and LSE in log2 units, into the workspace), the dQ pass and the separate
-// dK/dV pass -- one kernel template with two modes.  Deterministic: no atomics, every output
+// Item-axis attention backward on tcgen05: the dQ pass (which also
+// computes D = rowsum(dO o O) and -LSE*log2(e) per query row and leaves them in the workspace) and
+// the separate dK/dV pass -- one kernel template with two modes.  Deterministic: no atomics, every output
 // element has exactly one writer.  (The split costs one extra exp and two extra tile-matmuls per
 // (query, key) pair over a fused pass, but a fused pass must reduce dQ across key tiles with fp32
 // atomics: at dh = 32/64 that is 8-16 B of L2 atomic traffic per 10*dh flops -- see DESIGN.md.)
@@ -23,7 +23,11 @@
 //               pairs (+ the chunk's LSE/D vectors by 1-D bulk copy in MODE_DKV)
 //   warp 17     issuer of the score MMAs (S, dP), runs ahead of the accumulation as far as the two TMEM
 //               sets allow; owns the TMEM allocation
-//   warp 18     issuer of the acc0 MMAs (dQ or dV), warp 19 of the acc1 MMAs (dK, MODE_DKV only)
+//   warp 18     issuer of the acc0 MMAs (dQ or dV)
+//   warp 19     MODE_DKV: issuer of the acc1 MMAs (dK).  MODE_DQ: row statistics -- D_i = sum_k dO_ik O_ik
+//               from the item's dO tile and a TMA-staged O tile, -LSE_i*log2(e); handed to the score
+//               warpgroups through shared memory one item ahead, and written to the workspace for the
+//               dK/dV pass (this replaces a separate prep kernel: one pass less over O and dO)
 // Every role walks the same item list with its own counters.  The issuing warps run convergently with a
 // provably warp-uniform warp index, so ptxas keeps descriptors in uniform registers (~3 SASS instructions
 // per tcgen05.mma; the earlier builds needed ~10-20 and were bound by the issue chain,
@@ -37,9 +41,9 @@
 
 namespace tabattn {
 
-int item_bwd_padded_rows(const Shape& s);
-
 namespace {
+
+int item_bwd_padded_rows(const Shape& s);
 
 using namespace tc;
 using namespace itc;
@@ -60,7 +64,9 @@ struct BwdCfg {
   static constexpr int ST = DH >= 64 ? 8 : 16;
   static constexpr int LD_BYTES = 2 * kChunk * 4;  // per stage: lse2[64], D[64] (MODE_DKV)
   static constexpr int STAGE = 2 * TILE_B;         // bytes of one ring stage (B1, B2)
-  static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + 1024;
+  static constexpr int STAT_BYTES = 2 * 2 * kTileRows * 4;   // MODE_DQ: [2 item buffers][nlse2[128], D[128]]
+  // (+ one O tile in MODE_DQ; sized for the larger of the two modes)
+  static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + TILE_A + STAT_BYTES + 1024;
   // TMEM columns: set g at g*SET: S [0,64) dP [64,128) dS [128,160) P [160,192); accumulators after
   static constexpr int SET = 192, S_OFF = 0, DP_OFF = 64, DS_OFF = 128, P_OFF = 160;
   static constexpr int ACC0 = 384, ACC1 = 384 + DH, COLS = 512;
@@ -93,6 +99,12 @@ __device__ __forceinline__ Item decode_item(const Shape& s, const Meta& meta, in
   return it;
 }
 
+__device__ __forceinline__ uint4 lds_v4(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
+
 // 1-D bulk copy global -> shared, completion on an mbarrier (bytes multiple of 16, both 16 B aligned)
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -100,56 +112,13 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
                : "memory");
 }
 
-// ---- prep: D[b,c,h,r] = sum_k dO O, nlse2 = -LSE * log2(e); rows r in [R, Rp) get D = 0, nlse2 = -inf ----
-// One CTA = 32 rows of one (b, c); the two outputs are [B*C*H][Rp] f32 (Rp = R rounded up to 64).
-__global__ void __launch_bounds__(256) item_bwd_prep_kernel(Shape s, const __nv_bfloat16* __restrict__ O,
-                                                            const __nv_bfloat16* __restrict__ dO,
-                                                            const float* __restrict__ LSE,
-                                                            float* __restrict__ lse2_ws, float* __restrict__ D_ws,
-                                                            int Rp) {
-  __shared__ float sD[32][33];
-  const int bc = blockIdx.y, b = bc / s.C, c = bc - b * s.C;
-  if (s.col_valid && __ldg(s.col_valid + bc) == 0) return;
-  const int r0 = blockIdx.x * 32;
-  const int d = s.H * s.dh, vpr = d / 8, vph = s.dh / 8;
-  for (int i = threadIdx.x; i < 32 * 33; i += 256) (&sD[0][0])[i] = 0.f;
-  __syncthreads();
-  // 32 * vpr is a multiple of 32, so whole warps enter or leave the loop together (the shuffles below
-  // need every lane); rows >= R contribute 0 instead of branching around them.
-  for (int idx = threadIdx.x; idx < 32 * vpr; idx += 256) {
-    const int rr = idx / vpr, v = idx - rr * vpr, r = r0 + rr;
-    float a = 0.f;
-    if (r < s.R) {
-      const size_t off = (((size_t)b * s.R + r) * s.C + c) * d + 8 * v;
-      float fo[8], fg[8];
-      unpack8(ldg_nc_v4(O + off), fo);
-      unpack8(ldg_nc_v4(dO + off), fg);
-#pragma unroll
-      for (int e = 0; e < 8; ++e) a = fmaf(fo[e], fg[e], a);
-    }
-    // the vph partial sums of one (row, head) sit in vph consecutive lanes (vpr is a multiple of
-    // vph = 2, 4 or 8): butterfly-add them, a fixed order
-    for (int o = 1; o < vph; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-    if ((v % vph) == 0) sD[rr][v / vph] = a;
-  }
-  __syncthreads();
-  for (int idx = threadIdx.x; idx < 32 * s.H; idx += 256) {
-    const int h = idx >> 5, rr = idx & 31, r = r0 + rr;
-    if (r >= Rp) continue;
-    const size_t seq = ((size_t)bc * s.H + h);
-    const bool in = r < s.R;
-    lse2_ws[seq * Rp + r] = in ? -__ldg(LSE + seq * s.R + r) * kLog2e : -INFINITY;
-    D_ws[seq * Rp + r] = in ? sD[rr][h] : 0.f;
-  }
-}
-
 template <int DH, int MODE>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_constant__ CUtensorMap mapA2,
-                   const __grid_constant__ CUtensorMap mapB1, const __grid_constant__ CUtensorMap mapB2, Shape s,
-                   const float* __restrict__ lse2_ws, const float* __restrict__ D_ws,
-                   __nv_bfloat16* __restrict__ out0, __nv_bfloat16* __restrict__ out1, int n_items,
-                   int blocks_per_seq, int Rp) {
+                   const __grid_constant__ CUtensorMap mapB1, const __grid_constant__ CUtensorMap mapB2,
+                   const __grid_constant__ CUtensorMap mapO, Shape s, const float* __restrict__ LSE,
+                   float* lse2_ws, float* D_ws, __nv_bfloat16* __restrict__ out0,
+                   __nv_bfloat16* __restrict__ out1, int n_items, int blocks_per_seq, int Rp) {
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE_A = Cfg::TILE_A, TILE_B = Cfg::TILE_B, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -157,8 +126,12 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   const uint32_t sA = sbase;                         // [2 item buffers][A1, A2][TILE_A]
   const uint32_t sB = sA + 4 * TILE_A;               // [ST][B1, B2][TILE_B]
   const uint32_t sLD = sB + ST * Cfg::STAGE;         // [ST][lse2[64], D[64]]
+  const uint32_t sO = sLD + ST * Cfg::LD_BYTES;      // MODE_DQ: the item's O tile (single buffer)
+  const uint32_t sStat = sO + TILE_A;                // MODE_DQ: [2][nlse2[128], D[128]]
   const float* sLD_ptr = reinterpret_cast<const float*>(smem_raw + (sLD - smem_u32(smem_raw)));
+  float* sStat_ptr = reinterpret_cast<float*>(smem_raw + (sStat - smem_u32(smem_raw)));
   __shared__ uint64_t bar_a_full[2], bar_a_empty[2], bar_b_full[ST], bar_b_empty[ST];
+  __shared__ uint64_t bar_o_full, bar_o_empty, bar_d_full[2], bar_d_empty[2];
   __shared__ uint64_t bar_s_full[2], bar_s_empty[2], bar_p_full[2], bar_p_empty[2], bar_acc_full, bar_acc_free;
   __shared__ uint32_t tmem_slot;
   __shared__ int32_t s_ntrain[kMetaTabs];
@@ -176,7 +149,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       mbar_init(smem_u32(&bar_s_empty[i]), 8);   // one arrive per warp of the set's two warpgroups
       mbar_init(smem_u32(&bar_p_full[i]), 8);
       mbar_init(smem_u32(&bar_p_empty[i]), kAccWarps(MODE));
+      mbar_init(smem_u32(&bar_d_full[i]), 1);
+      mbar_init(smem_u32(&bar_d_empty[i]), kScoreWarps);
     }
+    mbar_init(smem_u32(&bar_o_full), 1);
+    mbar_init(smem_u32(&bar_o_empty), 1);
     for (int i = 0; i < ST; ++i) {
       mbar_init(smem_u32(&bar_b_full[i]), 1);
       mbar_init(smem_u32(&bar_b_empty[i]), kAccWarps(MODE));
@@ -201,6 +178,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       tma_prefetch_desc(&mapA2);
       tma_prefetch_desc(&mapB1);
       tma_prefetch_desc(&mapB2);
+      if (MODE == MODE_DQ) tma_prefetch_desc(&mapO);
       uint32_t t = 0, k = 0;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
         const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
@@ -210,6 +188,12 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         mbar_arrive_expect_tx(a_full, 2 * TILE_A);
         tma_load_5d(sA + (2 * ab) * TILE_A, &mapA1, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
         tma_load_5d(sA + (2 * ab + 1) * TILE_A, &mapA2, a_full, 0, it.h, it.c, it.blk * kTileRows, it.b);
+        if (MODE == MODE_DQ) {
+          // the item's O rows, for the stats warp (single buffer: it is read out right after it lands)
+          mbar_wait<true>(smem_u32(&bar_o_empty), (k & 1) ^ 1);
+          mbar_arrive_expect_tx(smem_u32(&bar_o_full), TILE_A);
+          tma_load_5d(sO, &mapO, smem_u32(&bar_o_full), 0, it.h, it.c, it.blk * kTileRows, it.b);
+        }
         const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
         for (int j = 0; j < it.chunks; ++j, ++t) {
           const uint32_t st = t % ST, b_full = smem_u32(&bar_b_full[st]);
@@ -300,6 +284,61 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       }
       ++k;
     }
+  } else if (MODE == MODE_DQ && warp == kScoreWarps + 3) {
+    // ------------------------------------------------------------------ row statistics (MODE_DQ)
+    // D_i = sum_k dO_ik O_ik over the item's 128 query rows, from the dO tile (A2) and the O tile in shared
+    // memory: both tiles carry the same swizzle, so equal physical 16-byte chunks hold equal logical ones and
+    // the dot product needs no address arithmetic.  CH lanes share a row; rows >= R were zero-filled by the
+    // TMA (D = 0) and get nlse2 = -inf (P = 0).  Runs one item ahead of the score warpgroups.
+    constexpr int CH = DH / 8, RPI = 32 / CH;   // 16-byte chunks per row, rows per warp iteration
+    const int sub = lane / CH, ch = lane % CH;
+    uint32_t k = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+      if (!it.valid) continue;
+      const uint32_t ab = k & 1;
+      const size_t seq = ((size_t)it.b * s.C + it.c) * s.H + it.h;
+      float l[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int row = it.blk * kTileRows + lane + 32 * q;
+        l[q] = row < s.R ? __ldg(LSE + seq * s.R + row) : INFINITY;
+      }
+      mbar_wait(smem_u32(&bar_a_full[ab]), (k >> 1) & 1);
+      mbar_wait(smem_u32(&bar_o_full), k & 1);
+      mbar_wait(smem_u32(&bar_d_empty[ab]), ((k >> 1) & 1) ^ 1);
+      float* st = sStat_ptr + ab * (2 * kTileRows);
+      const uint32_t tG = sA + (2 * ab + 1) * TILE_A + ch * 16, tO = sO + ch * 16;
+#pragma unroll 4
+      for (int r0 = 0; r0 < kTileRows; r0 += RPI) {
+        const int row = r0 + sub;
+        float fo[8], fg[8];
+        unpack8(lds_v4(tO + row * ROWB), fo);
+        unpack8(lds_v4(tG + row * ROWB), fg);
+        float a = 0.f;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) a = fmaf(fo[e], fg[e], a);
+#pragma unroll
+        for (int o = 1; o < CH; o <<= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if (ch == 0) st[kTileRows + row] = a;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&bar_o_empty));
+#pragma unroll
+      for (int q = 0; q < 4; ++q) st[lane + 32 * q] = -l[q] * kLog2e;
+      __syncwarp();
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int rr = lane + 32 * q, row = it.blk * kTileRows + rr;
+        if (row < Rp) {
+          lse2_ws[seq * Rp + row] = st[rr];
+          D_ws[seq * Rp + row] = st[kTileRows + rr];
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&bar_d_full[ab]));
+      ++k;
+    }
   }
   } else {
     // -------------------------------------------------------------------- score warpgroups
@@ -373,7 +412,6 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
       const int row = it.blk * kTileRows + r;
       const size_t cell = (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
-      const size_t seq = (((size_t)it.b * s.C + it.c) * s.H + it.h) * Rp;
       if (!it.valid) {
         // invalid column, or (MODE_DKV) a key block entirely beyond the train rows: zeros
         if (row < s.R && c == 0) {
@@ -388,11 +426,15 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         }
         continue;
       }
-      // per-row constants of the dQ pass (rows >= R: nlse2 = -inf -> P = 0)
+      // per-row constants of the dQ pass, from the stats warp (rows >= R: nlse2 = -inf -> P = 0)
       float nlse2 = -INFINITY, Drow = 0.f;
-      if (MODE == MODE_DQ && row < Rp) {
-        nlse2 = __ldg(lse2_ws + seq + row);
-        Drow = __ldg(D_ws + seq + row);
+      if (MODE == MODE_DQ) {
+        const uint32_t db = kitem & 1;
+        mbar_wait(smem_u32(&bar_d_full[db]), (kitem >> 1) & 1);
+        nlse2 = sStat_ptr[db * (2 * kTileRows) + r];
+        Drow = sStat_ptr[db * (2 * kTileRows) + kTileRows + r];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bar_d_empty[db]));
       }
       const uint64_t nl = f2pack(nlse2, nlse2), dd = f2pack(Drow, Drow);
       const int chunks = it.chunks;
@@ -487,52 +529,49 @@ template <int DH>
 cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O, const void* dO,
                        const float* LSE, void* dQ, void* dK, void* dV, float* ws, cudaStream_t stream) {
   using Cfg = BwdCfg<DH>;
-  CUtensorMap q128, g128, k128, v128, q64, g64, k64, v64;
-  bool ok = make_cell_tensor_map(&q128, Q, s.B, s.R, s.C, s.H, DH, kTileRows) &&
-            make_cell_tensor_map(&g128, dO, s.B, s.R, s.C, s.H, DH, kTileRows) &&
-            make_cell_tensor_map(&k128, K, s.B, s.R, s.C, s.H, DH, kTileRows) &&
-            make_cell_tensor_map(&v128, V, s.B, s.R, s.C, s.H, DH, kTileRows) &&
-            make_cell_tensor_map(&q64, Q, s.B, s.R, s.C, s.H, DH, kChunk) &&
-            make_cell_tensor_map(&g64, dO, s.B, s.R, s.C, s.H, DH, kChunk) &&
-            make_cell_tensor_map(&k64, K, s.B, s.R, s.C, s.H, DH, kChunk) &&
-            make_cell_tensor_map(&v64, V, s.B, s.R, s.C, s.H, DH, kChunk);
+  const DeviceInfo* di = current_device();
+  if (!di) return cudaErrorInvalidDevice;
+  CUtensorMap q128, g128, o128, k128, v128, q64, g64, k64, v64;
+  auto map = [&](CUtensorMap* m, const void* base, int rows) {
+    return get_tensor_map(m, 0, base, s.B, s.R, s.C, s.H, DH, rows, 1);
+  };
+  const bool ok = map(&q128, Q, kTileRows) && map(&g128, dO, kTileRows) && map(&o128, O, kTileRows) &&
+                  map(&k128, K, kTileRows) && map(&v128, V, kTileRows) && map(&q64, Q, kChunk) &&
+                  map(&g64, dO, kChunk) && map(&k64, K, kChunk) && map(&v64, V, kChunk);
   if (!ok) return cudaErrorInvalidValue;
   auto kq = item_bwd_tc_kernel<DH, MODE_DQ>;
   auto kkv = item_bwd_tc_kernel<DH, MODE_DKV>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kq, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kkv, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static SmemAttr attr_q, attr_kv;
+  cudaError_t e = attr_q.ensure(kq, Cfg::SMEM, di->ordinal);
+  if (e == cudaSuccess) e = attr_kv.ensure(kkv, Cfg::SMEM, di->ordinal);
+  if (e != cudaSuccess) return e;
   const int Rp = item_bwd_padded_rows(s);
   float* lse2_ws = ws;
   float* D_ws = ws + (size_t)s.B * s.C * s.H * Rp;
-  item_bwd_prep_kernel<<<dim3(Rp / 32, s.B * s.C), 256, 0, stream>>>(s, (const __nv_bfloat16*)O,
-                                                                     (const __nv_bfloat16*)dO, LSE, lse2_ws, D_ws, Rp);
   const int bps = (s.R + kTileRows - 1) / kTileRows;
   const long long n_items = (long long)s.B * s.C * s.H * bps;
-  const int grid = (int)std::min<long long>(n_items, num_sms());
-  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, s, lse2_ws, D_ws, (__nv_bfloat16*)dQ, nullptr,
-                                               (int)n_items, bps, Rp);
-  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, s, lse2_ws, D_ws, (__nv_bfloat16*)dV,
-                                                (__nv_bfloat16*)dK, (int)n_items, bps, Rp);
-  count_launch(3);
+  const int grid = (int)std::min<long long>(n_items, di->num_sms);
+  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, o128, s, LSE, lse2_ws, D_ws,
+                                               (__nv_bfloat16*)dQ, nullptr, (int)n_items, bps, Rp);
+  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, o128, s, LSE, lse2_ws, D_ws,
+                                                (__nv_bfloat16*)dV, (__nv_bfloat16*)dK, (int)n_items, bps, Rp);
+  count_launch(2);
   return cudaGetLastError();
 }
-
-}  // namespace
-
-bool item_tc_bwd_supported(const Shape& s) { return s.dh == 16 || s.dh == 32 || s.dh == 64; }
 
 // rows of the per-sequence LSE/D workspace vectors: R rounded up to the 64-row chunk, so that every
 // chunk's vectors are one aligned 256-byte bulk copy
 int item_bwd_padded_rows(const Shape& s) { return (s.R + kChunk - 1) / kChunk * kChunk; }
 
-cudaError_t launch_item_bwd_tc(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
-                               const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
-                               cudaStream_t stream) {
+}  // namespace
+
+size_t item_bwd_workspace_bytes(const Shape& s) {
+  return (size_t)2 * s.B * s.C * s.H * item_bwd_padded_rows(s) * sizeof(float);
+}
+
+cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
+                            const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
+                            cudaStream_t stream) {
   switch (s.dh) {
     case 16: return launch_bwd<16>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, stream);
     case 32: return launch_bwd<32>(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, stream);

@@ -342,21 +342,20 @@ template <int DH>
 cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                        cudaStream_t stream) {
   using Cfg = FwdCfg<DH>;
+  const DeviceInfo* di = current_device();
+  if (!di) return cudaErrorInvalidDevice;
   CUtensorMap mq, mk, mv;
-  if (!make_cell_tensor_map(&mq, Q, s.B, s.R, s.C, s.H, DH, kTileRows) ||
-      !make_cell_tensor_map(&mk, K, s.B, s.R, s.C, s.H, DH, kTileRows) ||
-      !make_cell_tensor_map(&mv, V, s.B, s.R, s.C, s.H, DH, kTileRows))
+  if (!get_tensor_map(&mq, 0, Q, s.B, s.R, s.C, s.H, DH, kTileRows, 1) ||
+      !get_tensor_map(&mk, 0, K, s.B, s.R, s.C, s.H, DH, kTileRows, 1) ||
+      !get_tensor_map(&mv, 0, V, s.B, s.R, s.C, s.H, DH, kTileRows, 1))
     return cudaErrorInvalidValue;
   auto kern = item_fwd_tc_kernel<DH>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static SmemAttr attr;
+  cudaError_t e = attr.ensure(kern, Cfg::SMEM, di->ordinal);
+  if (e != cudaSuccess) return e;
   const int bps = (s.R + 2 * kTileRows - 1) / (2 * kTileRows);
   const long long n_items = (long long)s.B * s.C * s.H * bps;
-  const int grid = (int)std::min<long long>(n_items, num_sms());
+  const int grid = (int)std::min<long long>(n_items, di->num_sms);
   kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, (int)n_items, bps);
   count_launch();
   return cudaGetLastError();
@@ -364,23 +363,8 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
 
 }  // namespace
 
-int num_sms() {
-  static int n = []() {
-    int dev = 0, v = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
-    return v > 0 ? v : 148;
-  }();
-  return n;
-}
-
-bool item_tc_supported(const Shape& s) {
-  // the tensor-map path needs 16-byte aligned global strides (always true: dh >= 16 bf16) and fits
-  // every shape the ABI accepts; tiny problems also run here (one code path to validate)
-  return s.dh == 16 || s.dh == 32 || s.dh == 64;
-}
-
-cudaError_t launch_item_fwd_tc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                               cudaStream_t stream) {
+cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
+                            cudaStream_t stream) {
   switch (s.dh) {
     case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, stream);
     case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, stream);

@@ -5,10 +5,11 @@
 #include <stdint.h>
 
 #include "common.cuh"
+#include "device.h"
 
 namespace tabattn {
 
-// ---- feature axis (feature_simt.cu) -------------------------------------------------------------
+// ---- feature axis (feature_tc.cu) ---------------------------------------------------------------------
 cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                cudaStream_t stream);
 cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
@@ -16,15 +17,14 @@ cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, con
                                cudaStream_t stream);
 bool feature_shape_supported(const Shape& s);
 
-// ---- item axis ------------------------------------------------------------------------------------
-// D (rowsum(dO o O), [B,C,H,R] f32) lives in the caller's workspace.
+// ---- item axis (item_tc_fwd.cu, item_tc_bwd.cu) ---------------------------------------------------------
+// The backward's workspace holds two f32 arrays [B*C*H][Rp] (Rp = R rounded up to 64): -LSE*log2(e) and
+// D = rowsum(dO o O), written by the dQ pass and read by the dK/dV pass.  The forward needs none.
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                            void* ws, cudaStream_t stream);
-cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
-                            const void* dO, const float* LSE, void* dQ, void* dK, void* dV, void* ws,
                             cudaStream_t stream);
-size_t item_fwd_workspace_bytes(const Shape& s);
-int num_sms();  // SM count of the current device (cached)
+cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
+                            const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
+                            cudaStream_t stream);
 size_t item_bwd_workspace_bytes(const Shape& s);
 
 }  // namespace tabattn

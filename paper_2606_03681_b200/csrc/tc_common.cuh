@@ -253,8 +253,4 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 
 }  // namespace tc
 
-// ---- host side: CUtensorMap over a [B,R,C,H,dh] bf16 tensor, box = (dh, 1, 1, rows, 1) -----------------
-// Returns false if the driver entry point is unavailable or the encode fails.
-bool make_cell_tensor_map(CUtensorMap* map, const void* base, int B, int R, int C, int H, int dh, int box_rows);
-
 }  // namespace tabattn

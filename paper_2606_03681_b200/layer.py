@@ -73,8 +73,12 @@ def layer_fwd_bwd_host(feat_host, item_host, feat_dev, item_dev, out_host, n_tra
     downloaded while group k computes -- PCIe is full duplex and the copies dominate the step
     (2 x 1.1 GB against 2.5 ms of kernels at base).  On return the current stream has been made to wait
     for the last download, so events recorded on it bracket the whole step."""
-    B = buf.shape[0]
-    groups = max(1, min(groups, B))
+    B, R, C, H, _ = buf.shape
+    # table-group boundaries must keep every sliced buffer 16-byte aligned: the f32 LSE slices start at
+    # b0 * R*H*C * 4 bytes, so b0 is kept a multiple of 4 / gcd(R*H*C, 4)
+    import math
+    align = 4 // math.gcd(R * H * C, 4)
+    groups = max(1, min(groups, B // align if B >= align else 1))
     cur = torch.cuda.current_stream()
     if getattr(buf, "_side", None) is None:
         buf._side = (torch.cuda.Stream(), torch.cuda.Stream())
@@ -82,7 +86,8 @@ def layer_fwd_bwd_host(feat_host, item_host, feat_dev, item_dev, out_host, n_tra
     s_in.wait_stream(cur)     # the previous step's kernels are done with the staging buffers
     s_out.wait_stream(cur)
     h2d = d2h = 0
-    bounds = [(B * g // groups, B * (g + 1) // groups) for g in range(groups)]
+    cuts = sorted({min(B, (B * g // groups) // align * align) for g in range(groups)} | {B})
+    bounds = [(a, b) for a, b in zip(cuts[:-1], cuts[1:]) if b > a]
     for b0, b1 in bounds:
         with torch.cuda.stream(s_in):
             for src, dst in ((feat_host, feat_dev), (item_host, item_dev)):

@@ -7,7 +7,7 @@ import paper_2606_03681_b200 as tab
 from oracle import ref
 from workloads import bf16_bits_to_f64
 
-from helpers import FWD_REL_L2, FWD_MAXABS_FRAC, GRAD_REL_L2, LSE_TOL, rel_l2
+from helpers import FWD_REL_L2, FWD_MAXABS_FRAC, GRAD_REL_L2, LSE_TOL, rel_l2, check_grad_hard
 
 
 def to_dev(bits):
@@ -90,6 +90,9 @@ def check_parity(axis, inp, gpu, orc, n_train=None, col_valid=None, what=""):
         if name == "O":
             mx = np.abs(g[mask] - r[mask]).max() if mask.any() else 0.0
             assert mx <= FWD_MAXABS_FRAC * vmax, "%s O max-abs %.3e" % (what, mx)
+        else:
+            # per-sequence and per-element gates: feature sequences run along C (axis 2), item along R (axis 1)
+            check_grad_hard(name, g, r, 2 if axis == "feature" else 1, what)
     lse_g = gpu["LSE"].cpu().numpy().astype(np.float64)
     lse_r = orc["LSE"]
     if axis == "feature":      # [B,R,H,C]

@@ -58,7 +58,7 @@ def test_workspace_bytes(tab):
     assert tab.workspace_bytes(s, 7) == 0
 
 
-def _call_fwd(tab, fn, shape, ptrs=(16, 16, 16, 16, 16), ws=None, nws=0):
+def _call_fwd(tab, fn, shape, ptrs=(16, 32, 48, 64, 80), ws=None, nws=0):
     f = getattr(tab.lib(), fn)
     args = [ctypes.c_void_p(p) if p else None for p in ptrs]
     return f(ctypes.byref(shape) if shape is not None else None, *args, ws, nws, None)
@@ -76,8 +76,8 @@ def test_argument_errors_need_no_device(tab, fn):
         assert _call_fwd(tab, fn, s) == tab.ERR_INVALID_ARG
     s = tab.TabattnShape(2, 8, 4, 2, 24, 4096, None, None, 0.0)
     assert _call_fwd(tab, fn, s) == tab.ERR_UNSUPPORTED
-    assert _call_fwd(tab, fn, ok, ptrs=(0, 16, 16, 16, 16)) == tab.ERR_INVALID_ARG      # NULL Q
-    assert _call_fwd(tab, fn, ok, ptrs=(16, 16, 24, 16, 16)) == tab.ERR_INVALID_ARG     # misaligned V
+    assert _call_fwd(tab, fn, ok, ptrs=(0, 32, 48, 64, 80)) == tab.ERR_INVALID_ARG      # NULL Q
+    assert _call_fwd(tab, fn, ok, ptrs=(16, 32, 56, 64, 80)) == tab.ERR_INVALID_ARG     # misaligned V
     if fn == "tabattn_item_fwd":
         s = tab.TabattnShape(2, 8, 4, 2, 16, None, None, None, 0.0)                     # NULL n_train
         assert _call_fwd(tab, fn, s) == tab.ERR_INVALID_ARG
@@ -89,7 +89,7 @@ def test_argument_errors_need_no_device(tab, fn):
         assert _call_fwd(tab, fn, s) == tab.ERR_INVALID_ARG
         # a good host copy passes validation (NULL Q is then the first error, still before any launch)
         s = tab.TabattnShape(2, 8, 4, 2, 16, 4096, ntp, None, 0.0)
-        assert _call_fwd(tab, fn, s, ptrs=(0, 16, 16, 16, 16)) == tab.ERR_INVALID_ARG
+        assert _call_fwd(tab, fn, s, ptrs=(0, 32, 48, 64, 80)) == tab.ERR_INVALID_ARG
     else:
         s = tab.TabattnShape(2, 8, 129, 2, 16, None, None, None, 0.0)                   # C too large
         assert _call_fwd(tab, fn, s) == tab.ERR_UNSUPPORTED
@@ -98,9 +98,40 @@ def test_argument_errors_need_no_device(tab, fn):
 def test_item_bwd_workspace_is_checked(tab):
     s = tab.TabattnShape(2, 8, 4, 2, 16, 4096, None, None, 0.0)
     f = tab.lib().tabattn_item_bwd
-    p = ctypes.c_void_p(16)
-    assert f(ctypes.byref(s), p, p, p, p, p, p, p, p, p, None, 0, None) == tab.ERR_WORKSPACE
-    assert f(ctypes.byref(s), p, p, p, p, p, p, p, p, p, p, 8, None) == tab.ERR_WORKSPACE
+    p = [ctypes.c_void_p(16 * (i + 1)) for i in range(10)]
+    assert f(ctypes.byref(s), *p[:9], None, 0, None) == tab.ERR_WORKSPACE
+    assert f(ctypes.byref(s), *p[:9], p[9], 8, None) == tab.ERR_WORKSPACE
+
+
+def test_output_aliasing_is_rejected(tab):
+    """tabattn.h: no aliasing of an output with any other argument (equal pointers are detected)."""
+    s = tab.TabattnShape(2, 8, 4, 2, 16, 4096, None, None, 0.0)
+    for fn in ("tabattn_feature_fwd", "tabattn_item_fwd"):
+        assert _call_fwd(tab, fn, s, ptrs=(16, 32, 48, 16, 80)) == tab.ERR_INVALID_ARG     # O over Q
+    p = [ctypes.c_void_p(16 * (i + 1)) for i in range(10)]
+    for fn in ("tabattn_feature_bwd", "tabattn_item_bwd"):
+        f = getattr(tab.lib(), fn)
+        a = list(p[:9])
+        a[6] = a[0]                                                                         # dQ over Q
+        assert f(ctypes.byref(s), *a, p[9], 1 << 20, None) == tab.ERR_INVALID_ARG
+        a = list(p[:9])
+        a[8] = a[7]                                                                         # dV over dK
+        assert f(ctypes.byref(s), *a, p[9], 1 << 20, None) == tab.ERR_INVALID_ARG
+
+
+def test_documented_limits_match_the_implementation(tab):
+    """include/tabattn.h documents TABATTN_MAX_D and TABATTN_MAX_FEATURE_C; B*C has no limit of its own."""
+    hdr = open(os.path.join(ROOT, "include", "tabattn.h")).read()
+    max_d = int(re.search(r"#define TABATTN_MAX_D (\d+)", hdr).group(1))
+    max_c = int(re.search(r"#define TABATTN_MAX_FEATURE_C (\d+)", hdr).group(1))
+    ok = tab.TabattnShape(1, 8, 4, max_d // 16, 16, 4096, None, None, 0.0)
+    assert tab.workspace_bytes(ok, tab.OP_ITEM_BWD) > 0
+    bad = tab.TabattnShape(1, 8, 4, max_d // 16 + 1, 16, 4096, None, None, 0.0)
+    assert tab.workspace_bytes(bad, tab.OP_ITEM_BWD) == 0
+    wide = tab.TabattnShape(700, 8, 100, 2, 16, 4096, None, None, 0.0)     # B*C = 70000 > 65535
+    assert tab.workspace_bytes(wide, tab.OP_ITEM_BWD) > 0
+    assert _call_fwd(tab, "tabattn_feature_fwd", tab.TabattnShape(2, 8, max_c + 1, 2, 16, None, None, None, 0.0)) \
+        == tab.ERR_UNSUPPORTED
 
 
 def test_product_never_imports_the_oracle():

@@ -69,6 +69,9 @@ EDGE = [
     # B*C = 8960 > 8192 cells: the backward kernels read n_train / col_valid from global memory instead of
     # their shared-memory copy (item_tc_common.cuh: Meta)
     ("meta_global_path", 70, 16, 128, 1, 16, 9),
+    # many heads (the old prep kernel's per-head scratch overflowed at H >= 34)
+    ("many_heads_dh16", 1, 140, 2, 40, 16, 70),
+    ("many_heads_dh64", 1, 70, 2, 35, 64, 33),
 ]
 
 

@@ -15,9 +15,10 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 from workloads import get_config, draw_structure, make_call_inputs, bf16_bits_to_f64  # noqa: E402
-from helpers import FWD_REL_L2, FWD_MAXABS_FRAC, GRAD_REL_L2, LSE_TOL, rel_l2  # noqa: E402
+from helpers import FWD_REL_L2, FWD_MAXABS_FRAC, GRAD_REL_L2, LSE_TOL, rel_l2, check_grad_hard  # noqa: E402
 
-FULL = ["base", "feature_heavy", "long_item", "ragged"]
+# (config, layer): ragged is checked on the first and the last of its 12 layers (own seeded projections each)
+FULL = [("base", 0), ("feature_heavy", 0), ("long_item", 0), ("ragged", 0), ("ragged", 11)]
 N_RANDOM_ROWS = 24
 
 
@@ -52,8 +53,22 @@ def _check(name, g, r, tol, what):
     return e
 
 
-@pytest.mark.parametrize("name", FULL)
-def test_full_size_sampled_parity(name):
+def _poison(torch, L, n_train_h, col_valid):
+    """NaN at every position that must not influence an output (SURVEY.md §8(b) "Values at masked
+    positions"): all inputs at invalid columns; item K/V at rows >= n_train[b]."""
+    nan = float("nan")
+    for ax in ("feature", "item"):
+        if col_valid is not None:
+            bad = (col_valid == 0)[:, None, :, None, None]
+            for k in ("Q", "K", "V", "dO"):
+                L[ax][k].masked_fill_(bad, nan)
+    for b, n in enumerate(n_train_h):
+        L["item"]["K"][b, int(n):] = nan
+        L["item"]["V"][b, int(n):] = nan
+
+
+@pytest.mark.parametrize("name,layer", FULL, ids=["%s-L%d" % f for f in FULL])
+def test_full_size_sampled_parity(name, layer):
     import torch
     import paper_2606_03681_b200 as tab
     from oracle import ref
@@ -63,8 +78,8 @@ def test_full_size_sampled_parity(name):
     n_train_h, col_valid_h = draw_structure(cfg)
     n_train = torch.from_numpy(n_train_h).to(dev)
     col_valid = torch.from_numpy(col_valid_h).to(dev) if col_valid_h is not None else None
-    layer = cfg.layers - 1      # ragged: the last of the 12 layers (its own seeded projections)
     L = {ax: make_call_inputs(cfg, ax, layer, device=dev) for ax in ("feature", "item")}
+    _poison(torch, L, n_train_h, col_valid)
     buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
     tab.layer_fwd_bwd(L["feature"], L["item"], n_train, col_valid, buf, n_train_h)
     torch.cuda.synchronize()
@@ -111,6 +126,7 @@ def test_full_size_sampled_parity(name):
         err = {"O": _check("O", g["O"], O, FWD_REL_L2, what)}
         for k, r in (("dQ", dQ), ("dK", dK), ("dV", dV)):
             err[k] = _check(k, g[k], r, GRAD_REL_L2, what)
+            check_grad_hard(k, g[k], r, 1, what)     # compact layout [n_sel, seq, H, dh]: the sequence is axis 1
         mx = np.abs(g["O"] - O).max()
         assert mx <= FWD_MAXABS_FRAC * vmax, "%s O max-abs %.3e > 1e-2 * %.3f" % (what, mx, vmax)
         lerr = np.abs(lg - LSE).max()
