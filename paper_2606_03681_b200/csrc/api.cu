@@ -106,13 +106,14 @@ size_t tabattn_workspace_bytes(const tabattn_shape* sh, int op) {
   if (check_shape(&tmp, op >= 2, &s) != TABATTN_OK) return 0;
   switch (op) {
     case TABATTN_OP_ITEM_BWD: return tabattn::item_bwd_workspace_bytes(s);
+    case TABATTN_OP_FEATURE_FWD:
+    case TABATTN_OP_FEATURE_BWD: return tabattn::feature_workspace_bytes(s);
     default: return 0;
   }
 }
 
 tabattn_status tabattn_feature_fwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
                                    float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream) {
-  (void)ws; (void)ws_bytes;
   Shape s;
   tabattn_status st = check_shape(sh, false, &s);
   if (st != TABATTN_OK) return st;
@@ -122,8 +123,10 @@ tabattn_status tabattn_feature_fwd(const tabattn_shape* sh, const void* Q, const
     const void* const ins[] = {Q, K, V};
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
+  // the workspace is only touched when a column mask is given (per-table geometry, a0)
+  if (s.col_valid && (st = check_ws(tabattn::feature_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_feature_fwd(s, Q, K, V, O, LSE, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_feature_fwd(s, Q, K, V, O, LSE, ws, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_feature_bwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V,

@@ -951,7 +951,6 @@ Plan make_plan(const Shape& s, bool bwd) {
 
 }  // namespace
 
-bool feature_shape_supported(const Shape& s) { return s.C <= 128; }
 
 namespace {
 
@@ -991,31 +990,6 @@ bool plan_ok(const Shape& s, const Plan& pl) {
 }
 
 }  // namespace
-
-cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                               cudaStream_t stream) {
-  const Plan pl = make_plan(s, false);
-  if (!plan_ok(s, pl)) return cudaErrorInvalidValue;
-  // the forward is also specialised on the number of 16-key blocks a row can have: two-pass softmax for 2 or
-  // 3-4 blocks (KB = 2, 4), the one-pass online form (KB = 0) for one block and for more than four
-  const int kb = (s.C + 15) / 16;
-#define TABATTN_FWD_KB(DHV, NS)                                                                                   \
-  if (kb == 2) return launch_persistent(feature_fwd_mma_kernel<DHV, NS, 2>, pl, stream, q, k, v, o, LSE);         \
-  if (kb == 3 || kb == 4) return launch_persistent(feature_fwd_mma_kernel<DHV, NS, 4>, pl, stream, q, k, v, o, LSE); \
-  return launch_persistent(feature_fwd_mma_kernel<DHV, NS, 0>, pl, stream, q, k, v, o, LSE);
-  const unsigned char *q = (const unsigned char*)Q, *k = (const unsigned char*)K, *v = (const unsigned char*)V;
-  unsigned char* o = (unsigned char*)O;
-  switch (s.dh * 10 + pl.p.nstage) {
-    case 162: { TABATTN_FWD_KB(16, 2) }
-    case 163: { TABATTN_FWD_KB(16, 3) }
-    case 322: { TABATTN_FWD_KB(32, 2) }
-    case 323: { TABATTN_FWD_KB(32, 3) }
-    case 642: { TABATTN_FWD_KB(64, 2) }
-    case 643: { TABATTN_FWD_KB(64, 3) }
-    default: return cudaErrorInvalidValue;
-  }
-#undef TABATTN_FWD_KB
-}
 
 cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
                                const void* dO, const float* LSE, void* dQ, void* dK, void* dV,

@@ -11,11 +11,12 @@ namespace tabattn {
 
 // ---- feature axis (feature_tc.cu) ---------------------------------------------------------------------
 cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                               cudaStream_t stream);
+                               void* ws, cudaStream_t stream);
 cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
                                const void* dO, const float* LSE, void* dQ, void* dK, void* dV,
                                cudaStream_t stream);
 bool feature_shape_supported(const Shape& s);
+size_t feature_workspace_bytes(const Shape& s);   // masked calls: per-table geometry built by the a0 prep kernel
 
 // ---- item axis (item_tc_fwd.cu, item_tc_bwd.cu) ---------------------------------------------------------
 // The backward's workspace holds two f32 arrays [B*C*H][Rp] (Rp = R rounded up to 64): -LSE*log2(e) and
