@@ -132,7 +132,6 @@ tabattn_status tabattn_feature_fwd(const tabattn_shape* sh, const void* Q, const
 tabattn_status tabattn_feature_bwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V,
                                    const void* O, const void* dO, const float* LSE, void* dQ, void* dK, void* dV,
                                    void* ws, size_t ws_bytes, tabattn_stream stream) {
-  (void)ws; (void)ws_bytes;
   Shape s;
   tabattn_status st = check_shape(sh, false, &s);
   if (st != TABATTN_OK) return st;
@@ -143,8 +142,9 @@ tabattn_status tabattn_feature_bwd(const tabattn_shape* sh, const void* Q, const
     const void* const ins[] = {Q, K, V, O, dO, LSE};
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
+  if (s.col_valid && (st = check_ws(tabattn::feature_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_feature_bwd(s, Q, K, V, O, dO, LSE, dQ, dK, dV, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_feature_bwd(s, Q, K, V, O, dO, LSE, dQ, dK, dV, ws, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_item_fwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,

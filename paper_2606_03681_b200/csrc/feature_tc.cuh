@@ -108,6 +108,38 @@ struct TileWalk {
   }
 };
 
+// Tables without a valid column have no tiles; their outputs are defined as +0 (LSE 0).  Called in the kernel
+// prologue by `nthr` threads of every CTA (grid-strided over the launch).
+template <int NOUT>
+__device__ __forceinline__ void zero_dead_tables(const FeatParams& p, unsigned char* const (&out)[NOUT], float* lse,
+                                                 int tid, int nthr) {
+  if (!p.masked) return;
+  const size_t tab_bytes = (size_t)p.s.R * p.s.C * p.s.H * p.s.dh * 2;
+  const size_t tab_lse = (size_t)p.s.R * p.s.H * p.s.C;
+  const size_t first = (size_t)blockIdx.x * nthr + tid, stride = (size_t)gridDim.x * nthr;
+  for (int b = 0; b < p.s.B; ++b) {
+    if (__ldg(&p.tabs[b].Cv) != 0) continue;
+    for (size_t i = first * 16; i < tab_bytes; i += stride * 16)
+#pragma unroll
+      for (int k = 0; k < NOUT; ++k) stg_v4(out[k] + (size_t)b * tab_bytes + i, make_uint4(0, 0, 0, 0));
+    if (lse)
+      for (size_t i = first; i < tab_lse; i += stride) lse[(size_t)b * tab_lse + i] = 0.f;
+  }
+}
+
+// log2(Cp) of the tile `back` tiles before tile t of table b (masked tables; -1 if there is none): the
+// same table almost always, else the nearest earlier table that has tiles.
+__device__ __forceinline__ int lgcp_of_earlier_tile(const FeatParams& p, const FeatTab& tb, int b, int t, int back) {
+  const int tp = t - back;
+  if (tp < 0) return -1;
+  if (tp >= tb.tile0) return tb.lgCp;
+  for (int bb = b - 1; bb >= 0; --bb) {
+    const int4 v = __ldg(reinterpret_cast<const int4*>(p.tabs + bb));
+    if (tp >= v.z && tp < v.w) return v.y;
+  }
+  return -1;
+}
+
 // 16-byte-chunk swizzle of a [rows][ROWB] tile whose swizzle span is one row (the TMA / UMMA layout):
 // chunk index XOR bits [7, 7+log2(CH)) of the byte offset.
 template <int ROWB>

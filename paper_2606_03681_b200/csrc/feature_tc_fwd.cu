@@ -80,12 +80,13 @@ __global__ void __launch_bounds__(256) feature_prep_kernel(Shape s, FeatTab* __r
     if (lane == 0) {
       int lg = 4;
       while ((1 << lg) < Cv) ++lg;
-      if (Cv == 0) lg = 7;                           // zero-fill only: one table row per tile
       const int rpt = kSlots >> lg;
       tabs[b].Cv = Cv;
       tabs[b].lgCp = lg;
       tabs[b].tile0 = 0;
-      tabs[b].tile1 = ((s.R + rpt - 1) / rpt) * s.H;   // tile count; turned into a range below
+      // tile count, turned into a range below; a table without a valid column has none (its outputs are
+      // zero-filled in the kernels' prologue)
+      tabs[b].tile1 = Cv == 0 ? 0 : ((s.R + rpt - 1) / rpt) * s.H;
     }
   }
   __syncthreads();
@@ -344,6 +345,10 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
     const uint32_t b_s_full = smem_u32(&bar_s_full[g]), b_p_full = smem_u32(&bar_p_full[g]),
                    b_pv_done = smem_u32(&bar_pv_done[g]);
     const float c2 = s.scale * kLog2e;
+    {
+      unsigned char* const outs[1] = {O};
+      zero_dead_tables<1>(p, outs, LSE, threadIdx.x, Cfg::SM_WARPS * 32);
+    }
     // per-thread constants of the staging path
     uint32_t st_off[DH / 8];
 #pragma unroll
@@ -463,6 +468,42 @@ int ceil_log2_min16(int c) {
   return lg;
 }
 
+}  // namespace
+
+// Geometry of one feature call.  Unmasked: one virtual table of B*R rows.  Masked: the a0 prep kernel builds the
+// per-table records in the workspace.  `lg` = log2 of the slots per row the TMA boxes are built for (unmasked).
+void feature_fill_params(const Shape& s, void* ws, cudaStream_t stream, ftc::FeatParams* pp, long long* max_tiles,
+                         int* lg_out) {
+  ftc::FeatParams& p = *pp;
+  p = ftc::FeatParams{};
+  p.s = s;
+  p.masked = s.col_valid != nullptr;
+  int lg = ceil_log2_min16(s.C);
+  if (p.masked) {
+    p.nTab = s.B;
+    p.Rt = s.R;
+    ftc::FeatTab* tabs = static_cast<ftc::FeatTab*>(ws);
+    uint8_t* vcol = reinterpret_cast<uint8_t*>(tabs + s.B);
+    int32_t* total = reinterpret_cast<int32_t*>(vcol + (size_t)s.B * 128);
+    p.tabs = tabs; p.vcol = vcol; p.total = total;
+    feature_prep_kernel<<<1, 256, 0, stream>>>(s, tabs, vcol, total);
+    count_launch();
+    *max_tiles = (long long)s.B * s.R * s.H;    // upper bound (Cp = 128: one row per tile)
+    lg = 7;                                     // (tensor maps unused)
+  } else {
+    const int rpt = ftc::kSlots >> lg;
+    const long long rows = (long long)s.B * s.R;
+    p.nTab = 1;
+    p.Rt = (int)rows;
+    p.n_tiles = (int)(((rows + rpt - 1) / rpt) * s.H);
+    p.uni.Cv = s.C; p.uni.lgCp = lg; p.uni.tile0 = 0; p.uni.tile1 = p.n_tiles;
+    *max_tiles = p.n_tiles;
+  }
+  *lg_out = lg;
+}
+
+namespace {
+
 template <int DH>
 cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE, void* ws,
                        cudaStream_t stream) {
@@ -470,30 +511,9 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
   const DeviceInfo* di = current_device();
   if (!di) return cudaErrorInvalidDevice;
   FeatParams p{};
-  p.s = s;
-  p.masked = s.col_valid != nullptr;
   long long max_tiles;
-  int lg = ceil_log2_min16(s.C);
-  if (p.masked) {
-    p.nTab = s.B;
-    p.Rt = s.R;
-    FeatTab* tabs = static_cast<FeatTab*>(ws);
-    uint8_t* vcol = reinterpret_cast<uint8_t*>(tabs + s.B);
-    int32_t* total = reinterpret_cast<int32_t*>(vcol + (size_t)s.B * 128);
-    p.tabs = tabs; p.vcol = vcol; p.total = total;
-    feature_prep_kernel<<<1, 256, 0, stream>>>(s, tabs, vcol, total);
-    count_launch();
-    max_tiles = (long long)s.B * s.R * s.H;    // upper bound (Cp = 128: one row per tile)
-    lg = 7;                                    // (tensor maps unused)
-  } else {
-    const int rpt = kSlots >> lg;
-    const long long rows = (long long)s.B * s.R;
-    p.nTab = 1;
-    p.Rt = (int)rows;
-    p.n_tiles = (int)(((rows + rpt - 1) / rpt) * s.H);
-    p.uni.Cv = s.C; p.uni.lgCp = lg; p.uni.tile0 = 0; p.uni.tile1 = p.n_tiles;
-    max_tiles = p.n_tiles;
-  }
+  int lg;
+  feature_fill_params(s, ws, stream, &p, &max_tiles, &lg);
   CUtensorMap mq, mk, mv, mo;
   const int rpt = kSlots >> lg;
   if (!get_tensor_map(&mq, 1, Q, s.B, s.R, s.C, s.H, DH, rpt, 1 << lg) ||

@@ -13,7 +13,7 @@ namespace tabattn {
 cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                void* ws, cudaStream_t stream);
 cudaError_t launch_feature_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
-                               const void* dO, const float* LSE, void* dQ, void* dK, void* dV,
+                               const void* dO, const float* LSE, void* dQ, void* dK, void* dV, void* ws,
                                cudaStream_t stream);
 bool feature_shape_supported(const Shape& s);
 size_t feature_workspace_bytes(const Shape& s);   // masked calls: per-table geometry built by the a0 prep kernel
