@@ -400,6 +400,8 @@ def run_ours(args):
     # ---- headline config: inputs resident in HBM before the timed region (replicas only across ranks:
     # each rank runs the same seeded workload on its own GPU)
     cfg = get_config(args.config)
+    if args.layers > 0:
+        cfg = cfg.scaled(layers=min(cfg.layers, args.layers))   # profiling runs: fewer layers resident
     wl = Workload(torch, tab, cfg, dev)
     m = time_workload(torch, dist, tab, wl, args.steps, args.warmup, args.min_region, world, rank, local, dev)
     work, call_ms = wl.work, m["call_ms"]
@@ -522,6 +524,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary configs")
     ap.add_argument("--cpu-budget", type=float, default=10.0)
+    ap.add_argument("--layers", type=int, default=0,
+                    help="keep only the first L layers of the config resident (ncu captures of ragged)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

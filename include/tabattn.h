@@ -103,6 +103,27 @@ TABATTN_API tabattn_status tabattn_item_bwd(const tabattn_shape* shape, const vo
                                 const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
                                 void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);
 
+/* ---- Forward-only evaluation path ----------------------------------------------
+ * evaluation tables hold at most 1000 rows x 100 features, 5-fold (800 train / 200 test
+ * rows); bf16 inference autocast; evaluation runs every 32-64 steps.
+ * Inference needs neither the saved log-sum-exp nor, in the last block, the outputs of the train rows
+ * ("the test-row outputs are sliced out"), so these calls write O only for the table rows
+ * [row0, row1) of EVERY table -- e.g. one chunk of test rows -- and no LSE.  Rows of O outside the range
+ * are not touched.  0 <= row0 < row1 <= R, else TABATTN_ERR_INVALID_ARG.  Everything else (layouts, the
+ * column mask, +0 at invalid columns, the train-only key rule) is as in the training forward, and the
+ * results on the range are bit-identical to it.
+ *
+ * Item: query rows [row0, row1) attend to the key rows [0, n_train[b]) of their own column; the caller
+ * passes the same K and V for every chunk of test rows (the train-row K/V are projected once and reused).
+ * Feature: the rows [row0, row1) of each table, each row alone.  A partial range with B > 1 is issued as
+ * one launch per table.  ws: tabattn_workspace_bytes(shape, TABATTN_OP_FEATURE_FWD / _ITEM_FWD). */
+TABATTN_API tabattn_status tabattn_feature_fwd_infer(const tabattn_shape* shape, const void* Q, const void* K,
+                                                     const void* V, void* O, int32_t row0, int32_t row1, void* ws,
+                                                     size_t ws_bytes, tabattn_stream stream);
+TABATTN_API tabattn_status tabattn_item_fwd_infer(const tabattn_shape* shape, const void* Q, const void* K,
+                                                  const void* V, void* O, int32_t row0, int32_t row1, void* ws,
+                                                  size_t ws_bytes, tabattn_stream stream);
+
 /* Bytes of device scratch `op` needs for `shape` (0 if shape is NULL or invalid). */
 TABATTN_API size_t tabattn_workspace_bytes(const tabattn_shape* shape, int op);
 

@@ -22,7 +22,7 @@ OP_FEATURE_FWD, OP_FEATURE_BWD, OP_ITEM_FWD, OP_ITEM_BWD = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, 1, 2, 3, 4
 
 EXPORTS = ("tabattn_feature_fwd", "tabattn_feature_bwd", "tabattn_item_fwd", "tabattn_item_bwd",
-           "tabattn_workspace_bytes", "tabattn_status_string", "tabattn_version", "tabattn_launch_count")
+           "tabattn_feature_fwd_infer", "tabattn_item_fwd_infer", "tabattn_workspace_bytes", "tabattn_status_string", "tabattn_version", "tabattn_launch_count")
 
 
 class TabattnShape(ctypes.Structure):
@@ -56,7 +56,11 @@ def lib():
         L.tabattn_item_fwd.argtypes = [shp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.tabattn_feature_bwd.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.tabattn_item_bwd.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
-        for f in (L.tabattn_feature_fwd, L.tabattn_item_fwd, L.tabattn_feature_bwd, L.tabattn_item_bwd):
+        i32 = ctypes.c_int32
+        L.tabattn_feature_fwd_infer.argtypes = [shp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
+        L.tabattn_item_fwd_infer.argtypes = [shp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
+        for f in (L.tabattn_feature_fwd, L.tabattn_item_fwd, L.tabattn_feature_bwd, L.tabattn_item_bwd,
+                  L.tabattn_feature_fwd_infer, L.tabattn_item_fwd_infer):
             f.restype = ctypes.c_int
         L.tabattn_workspace_bytes.argtypes = [shp, ctypes.c_int]
         L.tabattn_workspace_bytes.restype = sz
@@ -233,3 +237,34 @@ def tabattn_item_bwd(Q, K, V, O, dO, LSE, n_train, col_valid=None, softmax_scale
                                     _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_item_bwd")
     return dQ, dK, dV
+
+
+def tabattn_feature_fwd_infer(Q, K, V, row0, row1, col_valid=None, softmax_scale=0.0, O=None, ws=None, stream=None):
+    """Forward-only feature attention on the table rows [row0, row1), no LSE (tabattn.h:
+    tabattn_feature_fwd_infer).  Returns O; rows outside the range are left as they were."""
+    _check_inputs(Q, K, V, O)
+    _check_aux(Q, None, col_valid)
+    shape, keep = make_shape(Q, None, col_valid, None, softmax_scale)
+    O = torch.empty_like(Q) if O is None else O
+    ws, nws = _workspace(shape, OP_FEATURE_FWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_feature_fwd_infer(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), int(row0),
+                                             int(row1), _ptr(ws), nws, _stream(stream, Q.device))
+    _raise(st, "tabattn_feature_fwd_infer")
+    return O
+
+
+def tabattn_item_fwd_infer(Q, K, V, n_train, row0, row1, col_valid=None, softmax_scale=0.0, n_train_host=None,
+                           O=None, ws=None, stream=None):
+    """Forward-only item attention: query rows [row0, row1) against the train rows, no LSE (tabattn.h:
+    tabattn_item_fwd_infer).  Returns O; rows outside the range are left as they were."""
+    _check_inputs(Q, K, V, O)
+    _check_aux(Q, n_train, col_valid)
+    shape, keep = make_shape(Q, n_train, col_valid, n_train_host, softmax_scale)
+    O = torch.empty_like(Q) if O is None else O
+    ws, nws = _workspace(shape, OP_ITEM_FWD, ws, Q.device)
+    with _on(Q.device):
+        st = lib().tabattn_item_fwd_infer(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), int(row0),
+                                          int(row1), _ptr(ws), nws, _stream(stream, Q.device))
+    _raise(st, "tabattn_item_fwd_infer")
+    return O

@@ -160,7 +160,40 @@ tabattn_status tabattn_item_fwd(const tabattn_shape* sh, const void* Q, const vo
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, 0, s.R, (cudaStream_t)stream));
+}
+
+tabattn_status tabattn_feature_fwd_infer(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
+                                         int32_t row0, int32_t row1, void* ws, size_t ws_bytes,
+                                         tabattn_stream stream) {
+  Shape s;
+  tabattn_status st = check_shape(sh, false, &s);
+  if (st != TABATTN_OK) return st;
+  if (!all_ok(Q, K, V, (const void*)O) || row0 < 0 || row1 <= row0 || row1 > s.R) return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {O};
+    const void* const ins[] = {Q, K, V};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  if (s.col_valid && (st = check_ws(tabattn::feature_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
+  if ((st = check_device()) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_feature_fwd_infer(s, Q, K, V, O, row0, row1, ws, (cudaStream_t)stream));
+}
+
+tabattn_status tabattn_item_fwd_infer(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
+                                      int32_t row0, int32_t row1, void* ws, size_t ws_bytes, tabattn_stream stream) {
+  Shape s;
+  tabattn_status st = check_shape(sh, true, &s);
+  if (st != TABATTN_OK) return st;
+  (void)ws; (void)ws_bytes;
+  if (!all_ok(Q, K, V, (const void*)O) || row0 < 0 || row1 <= row0 || row1 > s.R) return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {O};
+    const void* const ins[] = {Q, K, V};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  if ((st = check_device()) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, nullptr, row0, row1, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_item_bwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V,

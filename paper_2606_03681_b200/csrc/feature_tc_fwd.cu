@@ -419,7 +419,7 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           unsigned char* oz = O + ((size_t)(grow0 + r) * s.C + c) * d2 + (size_t)x.h * ROWB;
 #pragma unroll
           for (int q = 0; q < DH / 8; ++q) stg_v4(oz + 16 * q, make_uint4(0, 0, 0, 0));
-          LSE[((size_t)(grow0 + r) * s.H + x.h) * s.C + c] = 0.f;
+          if (LSE) LSE[((size_t)(grow0 + r) * s.H + x.h) * s.C + c] = 0.f;
         }
         if (x.Cv == 0) continue;
         if (x.b != cur_b) {
@@ -443,7 +443,7 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       if (pd_on) store_prev();
       // ---- this tile: LSE = (m + log2 l) ln 2 now, O = acc / l deferred
       const bool live = rl < x.nrows && v < x.Cv;
-      if (live) LSE[((size_t)(grow0 + rl) * s.H + x.h) * s.C + my_col] = (m + log2f(l)) * kLn2;
+      if (live && LSE) LSE[((size_t)(grow0 + rl) * s.H + x.h) * s.C + my_col] = (m + log2f(l)) * kLn2;
       pd_on = true; pd_live = live; pd_inv = 1.f / l; pd_h = x.h; pd_col = my_col;
       pd_row = p.masked ? grow0 + rl : grow0;
       ++k;
@@ -534,13 +534,38 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
 
 }  // namespace
 
+// bytes per table: FeatTab + vcol[128] + the tile total, so that a call on ONE table (the row-range inference path
+// launches per table) can use its own aligned slice of the same workspace
+constexpr size_t kFeatureWsPerTable = sizeof(ftc::FeatTab) + 128 + 16;
+
 size_t feature_workspace_bytes(const Shape& s) {
   // FeatTab[B] + vcol[B][128] + total, for masked calls (sized without looking at col_valid, so that one
   // workspace serves both)
-  return (size_t)s.B * (sizeof(ftc::FeatTab) + 128) + 16;
+  return (size_t)s.B * kFeatureWsPerTable;
 }
 
 bool feature_shape_supported(const Shape& s) { return s.C <= 128; }
+
+// Forward-only inference on the table rows [row0, row1): feature attention treats every row
+// alone, so a row range is the same kernel on a sub-tensor -- one launch per table (the range of table b starts
+// (b R + row0) C d elements into the tensors); the whole range is one launch.  No LSE.
+cudaError_t launch_feature_fwd_infer(const Shape& s, const void* Q, const void* K, const void* V, void* O, int row0,
+                                     int row1, void* ws, cudaStream_t stream) {
+  if (row0 == 0 && row1 == s.R) return launch_feature_fwd(s, Q, K, V, O, nullptr, ws, stream);
+  const size_t cell = (size_t)s.C * s.H * s.dh * 2;
+  for (int b = 0; b < s.B; ++b) {
+    Shape t = s;
+    t.B = 1;
+    t.R = row1 - row0;
+    if (s.col_valid) t.col_valid = s.col_valid + (size_t)b * s.C;
+    const size_t off = ((size_t)b * s.R + row0) * cell;
+    cudaError_t e = launch_feature_fwd(t, (const char*)Q + off, (const char*)K + off, (const char*)V + off,
+                                       (char*)O + off, nullptr, ws ? (char*)ws + b * kFeatureWsPerTable : nullptr,
+                                       stream);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
 
 cudaError_t launch_feature_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                                void* ws, cudaStream_t stream) {

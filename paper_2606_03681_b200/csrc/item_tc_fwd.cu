@@ -49,7 +49,7 @@ template <int DH>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                    const __grid_constant__ CUtensorMap mapV, Shape s, __nv_bfloat16* __restrict__ O,
-                   float* __restrict__ LSE, int n_items, int blocks_per_seq) {
+                   float* __restrict__ LSE, int n_items, int blocks_per_seq, int q_row0, int q_row1) {
   using Cfg = FwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE = Cfg::TILE, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -100,7 +100,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const int qb = wk.k & 1;
             mbar_wait<true>(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
             mbar_arrive_expect_tx(smem_u32(&bar_q_full[qb]), 2 * TILE);
-            const int q0 = wk.blk * 2 * kTileRows;
+            const int q0 = q_row0 + wk.blk * 2 * kTileRows;
             tma_load_5d(sQ + (2 * qb) * TILE, &mapQ, smem_u32(&bar_q_full[qb]), 0, wk.h, wk.c, q0, wk.b);
             tma_load_5d(sQ + (2 * qb + 1) * TILE, &mapQ, smem_u32(&bar_q_full[qb]), 0, wk.h, wk.c, q0 + kTileRows,
                         wk.b);
@@ -232,14 +232,14 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     for (; it.ic.w < n_items; it.ic.next()) {
       bool valid;
       it.decode(s, valid);
-      const int row = it.blk * 2 * kTileRows + t * kTileRows + r;
+      const int row = q_row0 + it.blk * 2 * kTileRows + t * kTileRows + r;
       __nv_bfloat16* orow = O + (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
       float* lse = LSE + (((size_t)it.b * s.C + it.c) * s.H + it.h) * s.R + row;
       if (!valid) {
-        if (row < s.R) {
+        if (row < q_row1) {
 #pragma unroll
           for (int k = 0; k < DH / 8; ++k) stg_v4(orow + 8 * k, make_uint4(0, 0, 0, 0));
-          *lse = 0.f;
+          if (LSE) *lse = 0.f;
         }
         continue;
       }
@@ -320,7 +320,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       uint32_t o[DH];
       tmem_ld_cols<DH>(tO, o);
       tc_fence_before();
-      if (row < s.R) {
+      if (row < q_row1) {
         const float inv = 1.f / l;
 #pragma unroll
         for (int k = 0; k < DH / 8; ++k) {
@@ -329,7 +329,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(o[8 * k + e]) * inv;
           stg_v4(orow + 8 * k, pack8(f));
         }
-        *lse = (m + log2f(l)) * kLn2;
+        if (LSE) *lse = (m + log2f(l)) * kLn2;
       }
     }
   }
@@ -340,7 +340,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 
 template <int DH>
 cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                       cudaStream_t stream) {
+                       int q_row0, int q_row1, cudaStream_t stream) {
   using Cfg = FwdCfg<DH>;
   const DeviceInfo* di = current_device();
   if (!di) return cudaErrorInvalidDevice;
@@ -353,10 +353,12 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
   static SmemAttr attr;
   cudaError_t e = attr.ensure(kern, Cfg::SMEM, di->ordinal);
   if (e != cudaSuccess) return e;
-  const int bps = (s.R + 2 * kTileRows - 1) / (2 * kTileRows);
+  // query rows [q_row0, q_row1) of every sequence (the training forward passes [0, R)); keys are always [0, n_train)
+  const int bps = (q_row1 - q_row0 + 2 * kTileRows - 1) / (2 * kTileRows);
   const long long n_items = (long long)s.B * s.C * s.H * bps;
   const int grid = (int)std::min<long long>(n_items, di->num_sms);
-  kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, (int)n_items, bps);
+  kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, (int)n_items, bps, q_row0,
+                                                 q_row1);
   count_launch();
   return cudaGetLastError();
 }
@@ -364,11 +366,11 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
 }  // namespace
 
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                            cudaStream_t stream) {
+                            int q_row0, int q_row1, cudaStream_t stream) {
   switch (s.dh) {
-    case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, stream);
-    case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, stream);
-    case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, stream);
+    case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
+    case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
+    case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
     default: return cudaErrorInvalidValue;
   }
 }
