@@ -127,6 +127,54 @@ __device__ __forceinline__ void zero_dead_tables(const FeatParams& p, unsigned c
   }
 }
 
+// Zero-fill (a6) of the INVALID columns of masked tables, by spare warps of every CTA while the other warps
+// compute: a cell's H heads are d2 contiguous bytes, so a warp clears whole cells with coalesced 16-byte stores
+// (the softmax warps used to clear 2 dh bytes per (cell, head) with an integer division per store).  The CTA's
+// `nzw` zero-fill warps (this one is `zw`) share the rows r = blockIdx.x, += gridDim.x of every table; four
+// independent (column lookup, store) groups per lane and iteration keep several stores in flight.
+// lse (forward): 0.0f at [b][r][h][invalid c].  Tables without a valid column are left to zero_dead_tables.
+template <int NOUT>
+__device__ __forceinline__ void zero_invalid_cells(const FeatParams& p, unsigned char* const (&out)[NOUT], float* lse,
+                                                   int lane, int zw, int nzw) {
+  if (!p.masked) return;
+  const Shape& s = p.s;
+  const uint32_t d2 = (uint32_t)s.H * s.dh * 2;
+  const uint32_t chunks = d2 >> 4;                                     // 16-byte chunks per cell (<= 512)
+  const uint32_t m_ch = (uint32_t)((0x100000000ull + chunks - 1) / chunks);   // i / chunks = umulhi(i, m_ch), i < 2^16
+  for (int b = 0; b < s.B; ++b) {
+    const int Cv = __ldg(&p.tabs[b].Cv), ninv = s.C - Cv;
+    if (Cv == 0 || ninv == 0) continue;
+    const uint8_t* inv = p.vcol + (size_t)b * 128 + Cv;
+    const uint32_t total = (uint32_t)ninv * chunks;                    // <= 128 * 512
+    const uint32_t m_ni = (uint32_t)((0x100000000ull + ninv - 1) / ninv);
+    for (int r = blockIdx.x + zw * (int)gridDim.x; r < s.R; r += nzw * (int)gridDim.x) {
+      const size_t row = (size_t)b * s.R + r;
+      unsigned char* base[NOUT];
+#pragma unroll
+      for (int o = 0; o < NOUT; ++o) base[o] = out[o] + row * s.C * d2;
+      for (uint32_t i0 = lane; i0 < total; i0 += 128) {
+        uint32_t off[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const uint32_t i = i0 + 32 * u, k = __umulhi(i, m_ch), ch = i - k * chunks;
+          off[u] = i < total ? (uint32_t)__ldg(inv + k) * d2 + ch * 16 : 0xffffffffu;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (off[u] != 0xffffffffu) {
+#pragma unroll
+            for (int o = 0; o < NOUT; ++o) stg_v4(base[o] + off[u], make_uint4(0, 0, 0, 0));
+          }
+      }
+      if (lse)
+        for (uint32_t i = lane; i < (uint32_t)ninv * s.H; i += 32) {
+          const uint32_t h = __umulhi(i, m_ni), kk = i - h * ninv;
+          lse[(row * s.H + h) * s.C + __ldg(inv + kk)] = 0.f;
+        }
+    }
+  }
+}
+
 // log2(Cp) of the tile `back` tiles before tile t of table b (masked tables; -1 if there is none): the
 // same table almost always, else the nearest earlier table that has tiles.
 __device__ __forceinline__ int lgcp_of_earlier_tile(const FeatParams& p, const FeatTab& tb, int b, int t, int back) {

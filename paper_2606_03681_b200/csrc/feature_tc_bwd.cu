@@ -42,7 +42,8 @@ struct BwdCfg {
   static_assert(NSETS * SET <= COLS && 3 * DH <= SET, "TMEM budget");
   static constexpr int SM_WARPS = 4 * NSETS;
   static constexpr int PROD0 = SM_WARPS, SWARP = SM_WARPS + 4, DPWARP = SM_WARPS + 5, ACCWARP = SM_WARPS + 6;
-  static constexpr int WARPS = (SM_WARPS + 7 + 3) / 4 * 4;
+  static constexpr int ZWARP = SM_WARPS + 7;                 // zero-fill of invalid columns (masked tables)
+  static constexpr int WARPS = (SM_WARPS + 8 + 3) / 4 * 4;
   static constexpr int THREADS = WARPS * 32;
   static constexpr int REG_OTHER = DH >= 64 ? 72 : 56;
   static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
@@ -51,6 +52,7 @@ struct BwdCfg {
   static constexpr int NIN = 4;                        // Q, K, V, dO
   static constexpr int STAGE = NIN * TILE;
   static constexpr int ST = DH >= 64 ? 2 : (DH == 32 ? 4 : 6);
+  static constexpr int NLW = ST < 3 ? ST : 3;          // LSE-staging warps (unmasked tables)
   static constexpr int PDS = 2 * kSlots * 256;         // P and dS: [128][128] bf16 each
   static constexpr int SMEM = ST * STAGE + PDS + 2 * kMaskTile + 1024;
 };
@@ -81,13 +83,17 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
   __shared__ uint64_t bar_s_full[NSETS], bar_s_taken[NSETS], bar_dp_full[NSETS], bar_pds_full[NSETS],
       bar_acc_full[NSETS], bar_acc_free[NSETS];
   __shared__ uint32_t tmem_slot;
+  // -LSE log2(e) of every slot of a staged tile (+inf -> P = 0 for dead slots), written by the producer warps with
+  // the tile: the softmax threads used to fetch it themselves one tile ahead, which cost them a register they
+  // did not have (the value was spilled right behind the load: 19 % of their time, profiles/r02_feature.md)
+  __shared__ float sNL2[ST][kSlots];
   const Shape& s = p.s;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
   if (warp == Cfg::SWARP) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
   if (threadIdx.x == 0) {
     for (int i = 0; i < ST; ++i) {
-      mbar_init(smem_u32(&bar_full[i]), p.masked ? 128 : 1);
+      mbar_init(smem_u32(&bar_full[i]), p.masked ? 128 : 2);   // unmasked: the TMA lane + the tile's LSE warp
       mbar_init(smem_u32(&bar_empty[i]), 1);
     }
     for (int i = 0; i < NSETS; ++i) {
@@ -133,10 +139,46 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
             tma_load_4d(dst + 2 * TILE, &mapV, full, 0, x.h, 0, x.row0);
             tma_load_4d(dst + 3 * TILE, &mapG, full, 0, x.h, 0, x.row0);
           }
+        } else if (warp > Cfg::PROD0 && warp <= Cfg::PROD0 + Cfg::NLW) {
+          // LSE of the tiles n = j, j + NLW, ... (one of the other producer warps each), four slots per lane, fetched
+          // one own tile ahead of the stage wait.  NLW <= ST: a warp that strides further than the ring is deep
+          // could be two phases ahead of a stage's mbarrier, which a parity wait cannot tell from none.
+          constexpr int NLW = Cfg::NLW;
+          const int j = warp - Cfg::PROD0 - 1;
+          const int lg = p.uni.lgCp, Cv = p.uni.Cv, cm = (1 << lg) - 1;
+          float cur[4];
+          auto fetch = [&](const Tile& y, float (&v)[4]) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int slot = lane + 32 * q, rl = slot >> lg, c = slot & cm;
+              v[q] = (rl < y.nrows && c < Cv)
+                         ? __ldg(LSE + ((size_t)(y.row0 + rl) * s.H + y.h) * s.C + c) : INFINITY;
+            }
+          };
+          wk.init(p, j, NLW);
+          bool have = wk.get(p, x);
+          if (have) fetch(x, cur);
+          for (n = j; have; n += NLW) {
+            float nxt[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
+            wk.next(p);
+            Tile y;
+            have = wk.get(p, y);
+            if (have) fetch(y, nxt);
+            const uint32_t st = n % ST;
+            mbar_wait<true>(smem_u32(&bar_empty[st]), ((n / ST) & 1) ^ 1);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              sNL2[st][lane + 32 * q] = -cur[q] * kLog2e;
+              cur[q] = nxt[q];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&bar_full[st]));
+          }
         }
       } else {
         Gather<ROWB> ga;
         int cur_b = -1, pend = -1;
+        float pend_lse = INFINITY;
         for (wk.init(p); wk.get(p, x); wk.next(p), ++n) {
           if (x.b != cur_b) {
             cur_b = x.b;
@@ -150,14 +192,23 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           ga.issue(dst + 2 * TILE, V + g0, x.nrows);
           ga.issue(dst + 3 * TILE, dO + g0, x.nrows);
           cp_async_commit();
+          // the LSE of this lane's slot of the tile (stored when the stage is completed, an iteration later)
+          const int slot = (warp - Cfg::PROD0) * 32 + lane, rl = slot >> x.lgCp, v = slot & ((1 << x.lgCp) - 1);
+          float lse = INFINITY;
+          if (rl < x.nrows && v < x.Cv)
+            lse = __ldg(LSE + ((size_t)((size_t)x.b * s.R + x.row0 + rl) * s.H + x.h) * s.C +
+                        __ldg(p.vcol + (size_t)x.b * 128 + v));
           if (pend >= 0) {
+            sNL2[pend][slot] = -pend_lse * kLog2e;
             cp_async_wait<1>();
             fence_proxy_async_smem();
             mbar_arrive(smem_u32(&bar_full[pend]));
           }
           pend = (int)st;
+          pend_lse = lse;
         }
         if (pend >= 0) {
+          sNL2[pend][(warp - Cfg::PROD0) * 32 + lane] = -pend_lse * kLog2e;
           cp_async_wait<0>();
           fence_proxy_async_smem();
           mbar_arrive(smem_u32(&bar_full[pend]));
@@ -206,6 +257,10 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         }
         if (++g == NSETS) { g = 0; ++k; }
       }
+    } else if (warp >= Cfg::ZWARP) {
+      // ---------------------------------------------------------------------------- zero-fill of invalid columns (a6)
+      unsigned char* const outs[3] = {dQ, dK, dV};
+      zero_invalid_cells<3>(p, outs, nullptr, lane, warp - Cfg::ZWARP, Cfg::WARPS - Cfg::ZWARP);
     } else if (warp == Cfg::ACCWARP) {
       // ---------------------------------------------------------------------------- dQ = dS K, dK = dS^T Q, dV = P^T dO
       constexpr uint32_t idQ = make_idesc_bf16(128, DH, false, true);   // A K-major, B MN-major
@@ -267,44 +322,13 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
     Tile x;
     uint32_t k = 0;            // this set's tiles so far (= use index)
     int cur_b = -1, my_col = 0;
-    // raw LSE of the slot in this set's NEXT tile, fetched one tile ahead (a dead slot: +inf -> P = 0 in its row)
-    float lse_next = INFINITY;
-    auto fetch = [&](const Tile& y) {
-      lse_next = INFINITY;
-      const int yr = slot >> y.lgCp, yv = slot & ((1 << y.lgCp) - 1);
-      if (yr < y.nrows && yv < y.Cv) {
-        const int col = p.masked ? (int)__ldg(p.vcol + (size_t)y.b * 128 + yv) : yv;
-        const uint32_t row = (uint32_t)y.b * p.Rt + y.row0 + yr;
-        lse_next = __ldg(LSE + ((size_t)row * s.H + y.h) * s.C + col);
-      }
-    };
-    wk.init(p, g, NSETS);
-    if (wk.get(p, x)) fetch(x);
-    for (; wk.get(p, x); wk.next(p), ++k) {
+    for (wk.init(p, g, NSETS); wk.get(p, x); wk.next(p), ++k) {
       const int Cp = 1 << x.lgCp;
       const int rl = slot >> x.lgCp, v = slot & (Cp - 1);
       const uint32_t grow0 = (uint32_t)x.b * p.Rt + x.row0;
-      const float nl2 = -lse_next * kLog2e;
-      {
-        TileWalk nx = wk;     // (temporary: the next tile of this set, for the LSE prefetch)
-        Tile y;
-        nx.next(p);
-        if (nx.get(p, y)) fetch(y);
-      }
+      const uint32_t n = k * NSETS + g, st = n % ST;        // the tile's place in the CTA's walk, its stage
       int old_lg = x.lgCp;    // geometry the P/dS rows were last written with (the CTA's previous tile)
       if (p.masked) {
-        // zero-fill of the tile's invalid cells (a6): dQ, dK, dV := +0 at (row, invalid column, head h)
-        const int ninv = s.C - x.Cv;
-        for (int idx = slot; idx < x.nrows * ninv; idx += 128) {
-          const int r = idx / ninv, c = __ldg(p.vcol + (size_t)x.b * 128 + x.Cv + (idx - r * ninv));
-          const size_t zo = ((size_t)(grow0 + r) * s.C + c) * d2 + (size_t)x.h * ROWB;
-#pragma unroll
-          for (int q = 0; q < DH / 8; ++q) {
-            stg_v4(dQ + zo + 16 * q, make_uint4(0, 0, 0, 0));
-            stg_v4(dK + zo + 16 * q, make_uint4(0, 0, 0, 0));
-            stg_v4(dV + zo + 16 * q, make_uint4(0, 0, 0, 0));
-          }
-        }
         if (x.b != cur_b) {
           cur_b = x.b;
           my_col = v < x.Cv ? __ldg(p.vcol + (size_t)x.b * 128 + v) : 0;
@@ -316,7 +340,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       const bool live = rl < x.nrows && v < x.Cv;
       // the thread's window: its own block, or (Cp = 16) the two blocks of its warp
       const int colbase = x.lgCp >= 5 ? (((32 * wq) >> x.lgCp) << x.lgCp) : 32 * wq;
-      const uint64_t cc = f2pack(c2, c2), nl = f2pack(nl2, nl2);
+      const uint64_t cc = f2pack(c2, c2);
       const bool first_tile = g == 0 && k == 0;
 
       auto body = [&](auto WC) {
@@ -326,6 +350,11 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         // ---- pass A: P = 2^(S c2 - LSE log2e), packed bf16 pairs
         mbar_wait(b_s_full, k & 1);
         tc_fence_after();
+        // -LSE log2(e) of the slot, staged with the tile (the stage's barrier completed before the S MMA was issued;
+        // waiting on it here is what makes the producers' stores visible to this thread)
+        mbar_wait(smem_u32(&bar_full[st]), (n / ST) & 1);
+        const float nl2 = sNL2[st][slot];
+        const uint64_t nl = f2pack(nl2, nl2);
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
           uint32_t sr[32], pk[16];

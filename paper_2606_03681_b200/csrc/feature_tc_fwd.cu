@@ -6,12 +6,14 @@
 //                    slot reads its W = max(Cp, 32) score columns from TMEM, base-2 softmax (no running
 //                    maximum: a tile holds whole rows), writes P (bf16) back to TMEM; epilogue O / l -> bf16
 //                    through a staging tile and one TMA store (unmasked) or 16-byte stores to the gathered
-//                    columns (masked), LSE (natural log), zero-fill of invalid columns (a6)
+//                    columns (masked), LSE (natural log)
 //   warps 8-11       producer: unmasked -> one lane issues three TMA boxes per tile (Q, K, V);
 //                    masked -> all 128 lanes gather the valid cells with cp.async
 //   warp 12          issuer of S = Q K^T + mask bias (SS MMAs, fp32 in TMEM); owns the TMEM allocation and
 //                    rewrites the mask operands when the table geometry changes
 //   warp 13          issuer of O = P V (A = P from TMEM, B = the V tile MN-major)
+//   warps 14, 15     masked tables: zero-fill of the invalid columns (a6), whole cells, concurrently with the rest
+// (warp numbers for dh <= 32, three softmax warpgroups; dh = 64 has two)
 // TMEM: S0, S1 (128 columns each), P0, P1 (64 each: 128 bf16), O0, O1 (dh each).
 #include <cuda.h>
 
@@ -39,7 +41,7 @@ struct FwdCfg {
   static_assert(NSETS * SET <= COLS, "TMEM budget");
   static constexpr int SM_WARPS = 4 * NSETS;          // softmax warps
   static constexpr int PROD0 = SM_WARPS, SWARP = SM_WARPS + 4, PVWARP = SM_WARPS + 5;
-  static constexpr int WARPS = (SM_WARPS + 6 + 3) / 4 * 4;
+  static constexpr int WARPS = (SM_WARPS + 7 + 3) / 4 * 4;   // (+ the zero-fill warp)
   static constexpr int THREADS = WARPS * 32;
   static constexpr int REG_OTHER = DH >= 64 ? 72 : 56;
   // register pool = THREADS x (launch allocation, 65536 / THREADS rounded down to 8); what the other warps
@@ -307,6 +309,10 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         tc_commit_e(last_bar);
         ++ns;
       }
+    } else if (warp > Cfg::PVWARP) {
+      // ---------------------------------------------------------------------------- zero-fill of invalid columns (a6)
+      unsigned char* const outs[1] = {O};
+      zero_invalid_cells<1>(p, outs, LSE, lane, warp - Cfg::PVWARP - 1, Cfg::WARPS - Cfg::PVWARP - 1);
     } else if (warp == Cfg::PVWARP) {
       // ---------------------------------------------------------------------------- O = P V
       constexpr uint32_t idO = make_idesc_bf16(128, DH, false, true);
@@ -412,15 +418,6 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       const int rl = slot >> x.lgCp, v = slot & (Cp - 1);
       const uint32_t grow0 = (uint32_t)x.b * p.Rt + x.row0;   // first table row of the tile, global (< 2^31)
       if (p.masked) {
-        // zero-fill of the tile's invalid cells (a6): O := +0, LSE := 0 at (row, invalid column, head h)
-        const int ninv = s.C - x.Cv;
-        for (int idx = slot; idx < x.nrows * ninv; idx += 128) {
-          const int r = idx / ninv, c = __ldg(p.vcol + (size_t)x.b * 128 + x.Cv + (idx - r * ninv));
-          unsigned char* oz = O + ((size_t)(grow0 + r) * s.C + c) * d2 + (size_t)x.h * ROWB;
-#pragma unroll
-          for (int q = 0; q < DH / 8; ++q) stg_v4(oz + 16 * q, make_uint4(0, 0, 0, 0));
-          if (LSE) LSE[((size_t)(grow0 + r) * s.H + x.h) * s.C + c] = 0.f;
-        }
         if (x.Cv == 0) continue;
         if (x.b != cur_b) {
           cur_b = x.b;
