@@ -45,7 +45,7 @@ struct BwdCfg {
   static constexpr int ZWARP = SM_WARPS + 7;                 // zero-fill of invalid columns (masked tables)
   static constexpr int WARPS = (SM_WARPS + 8 + 3) / 4 * 4;
   static constexpr int THREADS = WARPS * 32;
-  static constexpr int REG_OTHER = DH >= 64 ? 72 : 56;
+  static constexpr int REG_OTHER = DH >= 64 ? 72 : 48;
   static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
   static constexpr int REG_SOFTMAX =
       ((THREADS * REG_LAUNCH - (WARPS - SM_WARPS) * 32 * REG_OTHER) / (SM_WARPS * 32)) / 8 * 8;
@@ -408,6 +408,45 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         f2unpack(dacc, d0, d1);
         const float D = d0 + d1;
         const uint64_t dd = f2pack(D, D);
+        // dS = P (dP - D) of one chunk (dr = the chunk's dP)
+        auto ds_chunk = [&](const uint32_t (&pk)[16], uint32_t (&ds)[16]) {
+#pragma unroll
+          for (int q = 0; q < 16; ++q) {
+            const uint64_t t = mul2(f2pack(bf16lo(pk[q]), bf16hi(pk[q])),
+                                    sub2(f2pack(__uint_as_float(dr[2 * q]), __uint_as_float(dr[2 * q + 1])), dd));
+            float a, b;
+            f2unpack(t, a, b);
+            ds[q] = pack_bf16(a, b);
+          }
+        };
+        auto store_chunk = [&](int c, const uint32_t (&pk)[16], const uint32_t (&ds)[16]) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int cj = colbase / 8 + 4 * c + q;
+            sts_v4(sP + pds_off(slot, cj), pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+            sts_v4(sDS + pds_off(slot, cj), ds[4 * q], ds[4 * q + 1], ds[4 * q + 2], ds[4 * q + 3]);
+          }
+        };
+        // The single P/dS buffer is the serial section of the kernel (a tile holds it from its first store to
+        // the completion of its accumulation MMAs), so everything that can be computed before the tile's turn
+        // is: for W <= 64 the dS chunks wait in registers and the turn only covers the stores
+        // (profiles/r02_feature.md: the turn wait was 20 % of the softmax warps' samples at base).
+        constexpr bool PRE = NCH <= 2;
+        uint32_t dsr[PRE ? 16 * NCH : 16];
+        if constexpr (PRE) {
+#pragma unroll
+          for (int c = 0; c < NCH; ++c) {
+            uint32_t pk[16], ds[16];
+            p_chunk(c, pk);
+            if (NCH > 1) {
+              tmem_ld32(tS + colbase + 32 * c, dr);
+              tmem_wait_ld();
+            }
+            ds_chunk(pk, ds);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) dsr[16 * c + q] = ds[q];
+          }
+        }
         // this tile's turn on the P/dS buffer
         if (!first_tile) mbar_wait(b_turn, (g == 0 ? k - 1 : k) & 1);
         if (old_lg >= 0 && old_lg != x.lgCp) {
@@ -423,24 +462,15 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         for (int c = 0; c < NCH; ++c) {
           uint32_t pk[16], ds[16];
           p_chunk(c, pk);
-          if (NCH > 1) {
+          if constexpr (PRE) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) ds[q] = dsr[16 * c + q];
+          } else {
             tmem_ld32(tS + colbase + 32 * c, dr);
             tmem_wait_ld();
+            ds_chunk(pk, ds);
           }
-#pragma unroll
-          for (int q = 0; q < 16; ++q) {
-            const uint64_t t = mul2(f2pack(bf16lo(pk[q]), bf16hi(pk[q])),
-                                    sub2(f2pack(__uint_as_float(dr[2 * q]), __uint_as_float(dr[2 * q + 1])), dd));
-            float a, b;
-            f2unpack(t, a, b);
-            ds[q] = pack_bf16(a, b);
-          }
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int cj = colbase / 8 + 4 * c + q;
-            sts_v4(sP + pds_off(slot, cj), pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
-            sts_v4(sDS + pds_off(slot, cj), ds[4 * q], ds[4 * q + 1], ds[4 * q + 2], ds[4 * q + 3]);
-          }
+          store_chunk(c, pk, ds);
         }
       };
       if (x.lgCp <= 5) body(std::integral_constant<int, 32>{});
