@@ -124,6 +124,74 @@ TABATTN_API tabattn_status tabattn_item_fwd_infer(const tabattn_shape* shape, co
                                                   const void* V, void* O, int32_t row0, int32_t row1, void* ws,
                                                   size_t ws_bytes, tabattn_stream stream);
 
+/* ---- The sub-blocks around the attention kernels ----------------------------
+ * PAPER.md:L69 (Fig. 3): every block applies feature-axis attention, sample-axis attention and an MLP, each
+ * with a norm; the norms sit BEFORE attention and MLP (pre-norm); RMSNorm;
+ * the input of block i is scaled by 0.95^i; explicit Q, K, V projections;
+ * MLP hidden width 768.  Where the paper is silent the readings b1-b6 of DESIGN.md §2
+ * apply: no biases; gain-only RMSNorm  xs rsqrt(mean(xs^2) + eps) o g  with statistics in fp32; exact (erf)
+ * GELU; weights stored [out][in] like nn.Linear; the decay factor alpha multiplies the sub-block's input.
+ *
+ *   attention sub-block:  xs = alpha x;  h = rmsnorm(xs) o g;  [q|k|v] = h Wqkv^T;  o = attention(q, k, v);
+ *                         y = xs + o Wo^T
+ *   MLP sub-block:        xs = alpha x;  h = rmsnorm(xs) o g;  u = h W1^T;  a = gelu(u);  y = xs + a W2^T
+ *
+ * x, y, dy, dx and every saved activation are bf16 [cells][e] (cells = B*R*C, the attention layout with
+ * e = H*dh) or [cells][hidden]; g is bf16 [e]; Wqkv [3e][e], Wo [e][e], W1 [hidden][e], W2 [e][hidden] bf16.
+ * Gradients of the parameters come back in fp32 (dg [e], dWqkv [3e][e], dWo [e][e], dW1, dW2), fully
+ * overwritten; they are reduced over the cells in a fixed order (no atomics: bitwise reproducible).
+ * The forward fills the `saved` buffers (caller-owned) the backward reads.  e must be a multiple of 64,
+ * e <= 1024, hidden a multiple of 64; alpha <= 0 means 1; eps <= 0 means 1e-6.
+ * axis: 0 = feature attention, 1 = item attention (shape->n_train required). */
+typedef struct {
+  void* h;      /* [cells][e] bf16    rmsnorm(alpha x) o g */
+  float* rstd;  /* [cells] f32        1 / sqrt(mean((alpha x)^2) + eps) */
+  void* q;      /* [cells][e] bf16 each: the projections and the attention output, in the attention layout */
+  void* k;
+  void* v;
+  void* o;
+  float* lse;   /* the attention's LSE (feature [B,R,H,C] / item [B,C,H,R]) */
+} tabattn_attn_saved;
+
+typedef struct {
+  void* h;      /* [cells][e] bf16 */
+  float* rstd;  /* [cells] f32 */
+  void* u;      /* [cells][hidden] bf16  pre-activation */
+  void* a;      /* [cells][hidden] bf16  gelu(u) */
+} tabattn_mlp_saved;
+
+TABATTN_API tabattn_status tabattn_attn_block_fwd(const tabattn_shape* shape, int32_t axis, float alpha, float eps,
+                                                  const void* x, const void* g, const void* Wqkv, const void* Wo,
+                                                  void* y, const tabattn_attn_saved* saved, void* ws,
+                                                  size_t ws_bytes, tabattn_stream stream);
+TABATTN_API tabattn_status tabattn_attn_block_bwd(const tabattn_shape* shape, int32_t axis, float alpha,
+                                                  const void* x, const void* g, const void* Wqkv, const void* Wo,
+                                                  const tabattn_attn_saved* saved, const void* dy, void* dx,
+                                                  float* dg, float* dWqkv, float* dWo, void* ws, size_t ws_bytes,
+                                                  tabattn_stream stream);
+/* scratch bytes of the two calls above (backward != 0: the backward's) */
+TABATTN_API size_t tabattn_attn_block_workspace_bytes(const tabattn_shape* shape, int32_t axis, int32_t backward);
+
+TABATTN_API tabattn_status tabattn_mlp_fwd(int64_t cells, int32_t e, int32_t hidden, float alpha, float eps,
+                                           const void* x, const void* g, const void* W1, const void* W2, void* y,
+                                           const tabattn_mlp_saved* saved, tabattn_stream stream);
+TABATTN_API tabattn_status tabattn_mlp_bwd(int64_t cells, int32_t e, int32_t hidden, float alpha, const void* x,
+                                           const void* g, const void* W1, const void* W2,
+                                           const tabattn_mlp_saved* saved, const void* dy, void* dx, float* dg,
+                                           float* dW1, float* dW2, void* ws, size_t ws_bytes,
+                                           tabattn_stream stream);
+TABATTN_API size_t tabattn_mlp_workspace_bytes(int64_t cells, int32_t e, int32_t hidden);
+
+/* Batched Newton-Schulz orthogonalisation, the core of the Muon update (PAPER.md:L85-87 Muon "with the same
+ * hyperparameters as in modded-nanogpt"; the iteration is batched across the QKV weight
+ * matrices).  For each of the nb matrices G_i [m][n] (bf16, m <= n):
+ *     X = G_i / (||G_i||_F + 1e-7);   `steps` times:  A = X X^T;  B = b A + c A A;  X = a X + B X
+ * with (a, b, c) = (3.4445, -4.7750, 2.0315), every product rounded to bf16 (reading b6).  X_out [nb][m][n]
+ * bf16.  m, n multiples of 8.  ws: tabattn_newton_schulz_workspace_bytes(nb, m, n). */
+TABATTN_API tabattn_status tabattn_newton_schulz(int32_t nb, int32_t m, int32_t n, const void* G, void* X_out,
+                                                 int32_t steps, void* ws, size_t ws_bytes, tabattn_stream stream);
+TABATTN_API size_t tabattn_newton_schulz_workspace_bytes(int32_t nb, int32_t m, int32_t n);
+
 /* Bytes of device scratch `op` needs for `shape` (0 if shape is NULL or invalid). */
 TABATTN_API size_t tabattn_workspace_bytes(const tabattn_shape* shape, int op);
 

@@ -22,7 +22,10 @@ OP_FEATURE_FWD, OP_FEATURE_BWD, OP_ITEM_FWD, OP_ITEM_BWD = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, 1, 2, 3, 4
 
 EXPORTS = ("tabattn_feature_fwd", "tabattn_feature_bwd", "tabattn_item_fwd", "tabattn_item_bwd",
-           "tabattn_feature_fwd_infer", "tabattn_item_fwd_infer", "tabattn_workspace_bytes", "tabattn_status_string", "tabattn_version", "tabattn_launch_count")
+           "tabattn_feature_fwd_infer", "tabattn_item_fwd_infer", "tabattn_workspace_bytes",
+           "tabattn_attn_block_fwd", "tabattn_attn_block_bwd", "tabattn_attn_block_workspace_bytes",
+           "tabattn_mlp_fwd", "tabattn_mlp_bwd", "tabattn_mlp_workspace_bytes",
+           "tabattn_newton_schulz", "tabattn_newton_schulz_workspace_bytes", "tabattn_status_string", "tabattn_version", "tabattn_launch_count")
 
 
 class TabattnShape(ctypes.Structure):
@@ -31,6 +34,16 @@ class TabattnShape(ctypes.Structure):
                 ("H", ctypes.c_int32), ("dh", ctypes.c_int32),
                 ("n_train", ctypes.c_void_p), ("n_train_host", ctypes.c_void_p),
                 ("col_valid", ctypes.c_void_p), ("softmax_scale", ctypes.c_float)]
+
+
+class TabattnAttnSaved(ctypes.Structure):
+    """Mirror of ``tabattn_attn_saved``."""
+    _fields_ = [(n, ctypes.c_void_p) for n in ("h", "rstd", "q", "k", "v", "o", "lse")]
+
+
+class TabattnMlpSaved(ctypes.Structure):
+    """Mirror of ``tabattn_mlp_saved``."""
+    _fields_ = [(n, ctypes.c_void_p) for n in ("h", "rstd", "u", "a")]
 
 
 class TabattnError(RuntimeError):
@@ -61,6 +74,22 @@ def lib():
         L.tabattn_item_fwd_infer.argtypes = [shp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
         for f in (L.tabattn_feature_fwd, L.tabattn_item_fwd, L.tabattn_feature_bwd, L.tabattn_item_bwd,
                   L.tabattn_feature_fwd_infer, L.tabattn_item_fwd_infer):
+            f.restype = ctypes.c_int
+        f32, i64 = ctypes.c_float, ctypes.c_int64
+        asv, msv = ctypes.POINTER(TabattnAttnSaved), ctypes.POINTER(TabattnMlpSaved)
+        L.tabattn_attn_block_fwd.argtypes = [shp, i32, f32, f32, vp, vp, vp, vp, vp, asv, vp, sz, vp]
+        L.tabattn_attn_block_bwd.argtypes = [shp, i32, f32, vp, vp, vp, vp, asv, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.tabattn_attn_block_workspace_bytes.argtypes = [shp, i32, i32]
+        L.tabattn_attn_block_workspace_bytes.restype = sz
+        L.tabattn_mlp_fwd.argtypes = [i64, i32, i32, f32, f32, vp, vp, vp, vp, vp, msv, vp]
+        L.tabattn_mlp_bwd.argtypes = [i64, i32, i32, f32, vp, vp, vp, vp, msv, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.tabattn_mlp_workspace_bytes.argtypes = [i64, i32, i32]
+        L.tabattn_mlp_workspace_bytes.restype = sz
+        L.tabattn_newton_schulz.argtypes = [i32, i32, i32, vp, vp, i32, vp, sz, vp]
+        L.tabattn_newton_schulz_workspace_bytes.argtypes = [i32, i32, i32]
+        L.tabattn_newton_schulz_workspace_bytes.restype = sz
+        for f in (L.tabattn_attn_block_fwd, L.tabattn_attn_block_bwd, L.tabattn_mlp_fwd, L.tabattn_mlp_bwd,
+                  L.tabattn_newton_schulz):
             f.restype = ctypes.c_int
         L.tabattn_workspace_bytes.argtypes = [shp, ctypes.c_int]
         L.tabattn_workspace_bytes.restype = sz
@@ -268,3 +297,139 @@ def tabattn_item_fwd_infer(Q, K, V, n_train, row0, row1, col_valid=None, softmax
                                           int(row1), _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_item_fwd_infer")
     return O
+
+
+# ---- sub-blocks (tabattn.h: "The sub-blocks around the attention kernels") ---------
+def _check_dense(t, dtype, shape, what):
+    if t.dtype != dtype or not t.is_cuda or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise ValueError("%s must be a contiguous CUDA %s tensor of shape %s" % (what, dtype, tuple(shape)))
+
+
+def _bytes_ws(need, ws, device):
+    if ws is None and need:
+        ws = torch.empty(need, dtype=torch.uint8, device=device)
+    return ws, (ws.numel() * ws.element_size() if ws is not None else 0)
+
+
+class AttnSaved:
+    """Caller-owned activations the attention sub-block's forward leaves for its backward."""
+
+    def __init__(self, x, H, axis):
+        B, R, C, e = x.shape
+        bf = dict(dtype=torch.bfloat16, device=x.device)
+        self.h, self.q, self.k, self.v, self.o = (torch.empty((B, R, C, e), **bf) for _ in range(5))
+        self.rstd = torch.empty((B * R * C,), dtype=torch.float32, device=x.device)
+        self.lse = torch.empty((B, R, H, C) if axis == 0 else (B, C, H, R), dtype=torch.float32, device=x.device)
+
+    def struct(self):
+        return TabattnAttnSaved(*[t.data_ptr() for t in (self.h, self.rstd, self.q, self.k, self.v, self.o, self.lse)])
+
+
+class MlpSaved:
+    def __init__(self, x, hidden):
+        cells, e = x.numel() // x.shape[-1], x.shape[-1]
+        bf = dict(dtype=torch.bfloat16, device=x.device)
+        self.h = torch.empty((cells, e), **bf)
+        self.u = torch.empty((cells, hidden), **bf)
+        self.a = torch.empty((cells, hidden), **bf)
+        self.rstd = torch.empty((cells,), dtype=torch.float32, device=x.device)
+
+    def struct(self):
+        return TabattnMlpSaved(*[t.data_ptr() for t in (self.h, self.rstd, self.u, self.a)])
+
+
+def _block_shape(x, H, n_train, col_valid, n_train_host):
+    B, R, C, e = x.shape
+    if e % H:
+        raise ValueError("e must be H * dh")
+    q5 = x.view(B, R, C, H, e // H)
+    _check_aux(q5, n_train, col_valid)
+    return make_shape(q5, n_train, col_valid, n_train_host, 0.0)
+
+
+def tabattn_attn_block_fwd(axis, x, g, Wqkv, Wo, H, n_train=None, col_valid=None, alpha=1.0, eps=1e-6,
+                           n_train_host=None, saved=None, y=None, ws=None, stream=None):
+    """Attention sub-block forward (tabattn.h: tabattn_attn_block_fwd).  x [B,R,C,e] bf16; axis 0 feature, 1 item.
+    Returns (y, saved)."""
+    B, R, C, e = x.shape
+    for t, shp, nm in ((x, x.shape, "x"), (g, (e,), "g"), (Wqkv, (3 * e, e), "Wqkv"), (Wo, (e, e), "Wo")):
+        _check_dense(t, torch.bfloat16, shp, nm)
+    shape, keep = _block_shape(x, H, n_train, col_valid, n_train_host)
+    saved = AttnSaved(x, H, axis) if saved is None else saved
+    y = torch.empty_like(x) if y is None else y
+    sv = saved.struct()
+    ws, nws = _bytes_ws(int(lib().tabattn_attn_block_workspace_bytes(ctypes.byref(shape), axis, 0)), ws, x.device)
+    with _on(x.device):
+        st = lib().tabattn_attn_block_fwd(ctypes.byref(shape), axis, float(alpha), float(eps), _ptr(x), _ptr(g),
+                                          _ptr(Wqkv), _ptr(Wo), _ptr(y), ctypes.byref(sv), _ptr(ws), nws,
+                                          _stream(stream, x.device))
+    _raise(st, "tabattn_attn_block_fwd")
+    return y, saved
+
+
+def tabattn_attn_block_bwd(axis, x, g, Wqkv, Wo, H, saved, dy, n_train=None, col_valid=None, alpha=1.0,
+                           n_train_host=None, ws=None, stream=None):
+    """Attention sub-block backward.  Returns (dx bf16, dg f32 [e], dWqkv f32 [3e,e], dWo f32 [e,e])."""
+    B, R, C, e = x.shape
+    _check_dense(dy, torch.bfloat16, x.shape, "dy")
+    shape, keep = _block_shape(x, H, n_train, col_valid, n_train_host)
+    f32 = dict(dtype=torch.float32, device=x.device)
+    dx, dg = torch.empty_like(x), torch.empty((e,), **f32)
+    dWqkv, dWo = torch.empty((3 * e, e), **f32), torch.empty((e, e), **f32)
+    sv = saved.struct()
+    ws, nws = _bytes_ws(int(lib().tabattn_attn_block_workspace_bytes(ctypes.byref(shape), axis, 1)), ws, x.device)
+    with _on(x.device):
+        st = lib().tabattn_attn_block_bwd(ctypes.byref(shape), axis, float(alpha), _ptr(x), _ptr(g), _ptr(Wqkv),
+                                          _ptr(Wo), ctypes.byref(sv), _ptr(dy), _ptr(dx), _ptr(dg), _ptr(dWqkv),
+                                          _ptr(dWo), _ptr(ws), nws, _stream(stream, x.device))
+    _raise(st, "tabattn_attn_block_bwd")
+    return dx, dg, dWqkv, dWo
+
+
+def tabattn_mlp_fwd(x, g, W1, W2, alpha=1.0, eps=1e-6, saved=None, y=None, stream=None):
+    """MLP sub-block forward (tabattn.h: tabattn_mlp_fwd).  x [..., e] bf16.  Returns (y, saved)."""
+    e, hidden = x.shape[-1], W1.shape[0]
+    cells = x.numel() // e
+    for t, shp, nm in ((x, x.shape, "x"), (g, (e,), "g"), (W1, (hidden, e), "W1"), (W2, (e, hidden), "W2")):
+        _check_dense(t, torch.bfloat16, shp, nm)
+    saved = MlpSaved(x, hidden) if saved is None else saved
+    y = torch.empty_like(x) if y is None else y
+    sv = saved.struct()
+    with _on(x.device):
+        st = lib().tabattn_mlp_fwd(cells, e, hidden, float(alpha), float(eps), _ptr(x), _ptr(g), _ptr(W1), _ptr(W2),
+                                   _ptr(y), ctypes.byref(sv), _stream(stream, x.device))
+    _raise(st, "tabattn_mlp_fwd")
+    return y, saved
+
+
+def tabattn_mlp_bwd(x, g, W1, W2, saved, dy, alpha=1.0, ws=None, stream=None):
+    """MLP sub-block backward.  Returns (dx bf16, dg f32 [e], dW1 f32 [hidden,e], dW2 f32 [e,hidden])."""
+    e, hidden = x.shape[-1], W1.shape[0]
+    cells = x.numel() // e
+    _check_dense(dy, torch.bfloat16, x.shape, "dy")
+    f32 = dict(dtype=torch.float32, device=x.device)
+    dx, dg = torch.empty_like(x), torch.empty((e,), **f32)
+    dW1, dW2 = torch.empty((hidden, e), **f32), torch.empty((e, hidden), **f32)
+    sv = saved.struct()
+    ws, nws = _bytes_ws(int(lib().tabattn_mlp_workspace_bytes(cells, e, hidden)), ws, x.device)
+    with _on(x.device):
+        st = lib().tabattn_mlp_bwd(cells, e, hidden, float(alpha), _ptr(x), _ptr(g), _ptr(W1), _ptr(W2),
+                                   ctypes.byref(sv), _ptr(dy), _ptr(dx), _ptr(dg), _ptr(dW1), _ptr(dW2), _ptr(ws), nws,
+                                   _stream(stream, x.device))
+    _raise(st, "tabattn_mlp_bwd")
+    return dx, dg, dW1, dW2
+
+
+def tabattn_newton_schulz(G, steps=5, X=None, ws=None, stream=None):
+    """Batched Newton-Schulz orthogonalisation (tabattn.h: tabattn_newton_schulz).  G [nb,m,n] bf16, m <= n."""
+    if G.dim() != 3:
+        raise ValueError("G must be [nb, m, n]")
+    nb, m, n = G.shape
+    _check_dense(G, torch.bfloat16, G.shape, "G")
+    X = torch.empty_like(G) if X is None else X
+    ws, nws = _bytes_ws(int(lib().tabattn_newton_schulz_workspace_bytes(nb, m, n)), ws, G.device)
+    with _on(G.device):
+        st = lib().tabattn_newton_schulz(nb, m, n, _ptr(G), _ptr(X), int(steps), _ptr(ws), nws,
+                                         _stream(stream, G.device))
+    _raise(st, "tabattn_newton_schulz")
+    return X

@@ -215,4 +215,136 @@ tabattn_status tabattn_item_bwd(const tabattn_shape* sh, const void* Q, const vo
                                             (cudaStream_t)stream));
 }
 
+// ---- sub-blocks -------------------------------------------------------------------
+
+namespace {
+bool block_dims_ok(int e, int hidden) { return e >= 64 && e <= 1024 && e % 64 == 0 && (hidden == 0 || (hidden >= 64 && hidden % 64 == 0)); }
+float or_default(float v, float d) { return v > 0.f ? v : d; }
+}  // namespace
+
+size_t tabattn_attn_block_workspace_bytes(const tabattn_shape* sh, int32_t axis, int32_t backward) {
+  Shape s;
+  if (!sh || (axis != 0 && axis != 1)) return 0;
+  tabattn_shape tmp = *sh;
+  static const int32_t dummy = 1;
+  if (!tmp.n_train) tmp.n_train = &dummy;
+  tmp.n_train_host = nullptr;
+  if (check_shape(&tmp, axis == 1, &s) != TABATTN_OK) return 0;
+  const tabattn::DeviceInfo* di = tabattn::current_device();
+  const int sms = di ? di->num_sms : 148;
+  return backward ? tabattn::attn_block_bwd_ws_bytes(s, axis, sms) : tabattn::feature_workspace_bytes(s);
+}
+
+tabattn_status tabattn_attn_block_fwd(const tabattn_shape* sh, int32_t axis, float alpha, float eps, const void* x,
+                                      const void* g, const void* Wqkv, const void* Wo, void* y,
+                                      const tabattn_attn_saved* sv, void* ws, size_t ws_bytes, tabattn_stream stream) {
+  Shape s;
+  if (axis != 0 && axis != 1) return TABATTN_ERR_INVALID_ARG;
+  tabattn_status st = check_shape(sh, axis == 1, &s);
+  if (st != TABATTN_OK) return st;
+  if (!block_dims_ok(s.H * s.dh, 0)) return TABATTN_ERR_UNSUPPORTED;
+  if (!sv || !all_ok(x, g, Wqkv, Wo, (const void*)y, (const void*)sv->h, (const void*)sv->rstd, (const void*)sv->q,
+                     (const void*)sv->k, (const void*)sv->v, (const void*)sv->o, (const void*)sv->lse))
+    return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {y, sv->h, sv->rstd, sv->q, sv->k, sv->v, sv->o, sv->lse};
+    const void* const ins[] = {x, g, Wqkv, Wo};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  if (axis == 0 && s.col_valid && (st = check_ws(tabattn::feature_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
+  if ((st = check_device()) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_attn_block_fwd(s, axis, or_default(alpha, 1.f), or_default(eps, 1e-6f), x, g, Wqkv,
+                                                  Wo, y, sv->h, sv->rstd, sv->q, sv->k, sv->v, sv->o, sv->lse, ws,
+                                                  (cudaStream_t)stream));
+}
+
+tabattn_status tabattn_attn_block_bwd(const tabattn_shape* sh, int32_t axis, float alpha, const void* x, const void* g,
+                                      const void* Wqkv, const void* Wo, const tabattn_attn_saved* sv, const void* dy,
+                                      void* dx, float* dg, float* dWqkv, float* dWo, void* ws, size_t ws_bytes,
+                                      tabattn_stream stream) {
+  Shape s;
+  if (axis != 0 && axis != 1) return TABATTN_ERR_INVALID_ARG;
+  tabattn_status st = check_shape(sh, axis == 1, &s);
+  if (st != TABATTN_OK) return st;
+  if (!block_dims_ok(s.H * s.dh, 0)) return TABATTN_ERR_UNSUPPORTED;
+  if (!sv || !all_ok(x, g, Wqkv, Wo, dy, (const void*)dx, (const void*)dg, (const void*)dWqkv, (const void*)dWo,
+                     (const void*)sv->h, (const void*)sv->rstd, (const void*)sv->q, (const void*)sv->k,
+                     (const void*)sv->v, (const void*)sv->o, (const void*)sv->lse))
+    return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {dx, dg, dWqkv, dWo, ws};
+    const void* const ins[] = {x, g, Wqkv, Wo, dy, sv->h, sv->rstd, sv->q, sv->k, sv->v, sv->o, sv->lse};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  if ((st = check_device()) != TABATTN_OK) return st;
+  const tabattn::DeviceInfo* di = tabattn::current_device();
+  if ((st = check_ws(tabattn::attn_block_bwd_ws_bytes(s, axis, di->num_sms), ws, ws_bytes)) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_attn_block_bwd(s, axis, or_default(alpha, 1.f), x, g, Wqkv, Wo, sv->h, sv->rstd,
+                                                  sv->q, sv->k, sv->v, sv->o, sv->lse, dy, dx, dg, dWqkv, dWo, ws,
+                                                  ws_bytes, (cudaStream_t)stream));
+}
+
+size_t tabattn_mlp_workspace_bytes(int64_t cells, int32_t e, int32_t hidden) {
+  if (cells < 1 || cells >= (1LL << 31) || !block_dims_ok(e, hidden) || hidden == 0) return 0;
+  const tabattn::DeviceInfo* di = tabattn::current_device();
+  return tabattn::block_ws_bytes(cells, e, hidden, di ? di->num_sms : 148);
+}
+
+tabattn_status tabattn_mlp_fwd(int64_t cells, int32_t e, int32_t hidden, float alpha, float eps, const void* x,
+                               const void* g, const void* W1, const void* W2, void* y, const tabattn_mlp_saved* sv,
+                               tabattn_stream stream) {
+  if (cells < 1) return TABATTN_ERR_INVALID_ARG;
+  if (cells >= (1LL << 31) || !block_dims_ok(e, hidden) || hidden == 0) return TABATTN_ERR_UNSUPPORTED;
+  if (!sv || !all_ok(x, g, W1, W2, (const void*)y, (const void*)sv->h, (const void*)sv->rstd, (const void*)sv->u,
+                     (const void*)sv->a))
+    return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {y, sv->h, sv->rstd, sv->u, sv->a};
+    const void* const ins[] = {x, g, W1, W2};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  tabattn_status st = check_device();
+  if (st != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_mlp_fwd(cells, e, hidden, or_default(alpha, 1.f), or_default(eps, 1e-6f), x, g, W1,
+                                           W2, y, sv->h, sv->rstd, sv->u, sv->a, (cudaStream_t)stream));
+}
+
+tabattn_status tabattn_mlp_bwd(int64_t cells, int32_t e, int32_t hidden, float alpha, const void* x, const void* g,
+                               const void* W1, const void* W2, const tabattn_mlp_saved* sv, const void* dy, void* dx,
+                               float* dg, float* dW1, float* dW2, void* ws, size_t ws_bytes, tabattn_stream stream) {
+  if (cells < 1) return TABATTN_ERR_INVALID_ARG;
+  if (cells >= (1LL << 31) || !block_dims_ok(e, hidden) || hidden == 0) return TABATTN_ERR_UNSUPPORTED;
+  if (!sv || !all_ok(x, g, W1, W2, dy, (const void*)dx, (const void*)dg, (const void*)dW1, (const void*)dW2,
+                     (const void*)sv->h, (const void*)sv->rstd, (const void*)sv->u, (const void*)sv->a))
+    return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {dx, dg, dW1, dW2, ws};
+    const void* const ins[] = {x, g, W1, W2, dy, sv->h, sv->rstd, sv->u, sv->a};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  tabattn_status st = check_device();
+  if (st != TABATTN_OK) return st;
+  if ((st = check_ws(tabattn_mlp_workspace_bytes(cells, e, hidden), ws, ws_bytes)) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_mlp_bwd(cells, e, hidden, or_default(alpha, 1.f), x, g, W1, W2, sv->h, sv->rstd,
+                                           sv->u, sv->a, dy, dx, dg, dW1, dW2, ws, ws_bytes, (cudaStream_t)stream));
+}
+
+size_t tabattn_newton_schulz_workspace_bytes(int32_t nb, int32_t m, int32_t n) {
+  if (nb < 1 || m < 8 || n < m || (m & 7) || (n & 7)) return 0;
+  return tabattn::newton_schulz_ws_bytes(nb, m, n);
+}
+
+tabattn_status tabattn_newton_schulz(int32_t nb, int32_t m, int32_t n, const void* G, void* X, int32_t steps, void* ws,
+                                     size_t ws_bytes, tabattn_stream stream) {
+  if (nb < 1 || m < 1 || n < 1 || steps < 0) return TABATTN_ERR_INVALID_ARG;
+  if (m < 8 || n < m || (m & 7) || (n & 7) || steps > 64) return TABATTN_ERR_UNSUPPORTED;
+  if (!all_ok(G, (const void*)X) || G == X) return TABATTN_ERR_INVALID_ARG;
+  tabattn_status st = check_ws(tabattn::newton_schulz_ws_bytes(nb, m, n), ws, ws_bytes);
+  if (st != TABATTN_OK) return st;
+  if ((st = check_device()) != TABATTN_OK) return st;
+  // Muon's quintic coefficients (Jordan et al. 2024b, as in modded-nanogpt)
+  return from_cuda(tabattn::launch_newton_schulz(nb, m, n, G, X, steps, 3.4445f, -4.7750f, 2.0315f, 1e-7f, ws,
+                                                 (cudaStream_t)stream));
+}
+
 }  // extern "C"

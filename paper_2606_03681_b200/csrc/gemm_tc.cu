@@ -1,0 +1,381 @@
+// tcgen05 GEMM core (gemm_tc.cuh): one 128 x BN output tile per CTA, a 4-stage TMA ring over 64-wide k-blocks,
+// fp32 accumulator in TMEM, fused epilogue, TMA store.  Warp 0 = TMA producer (one lane), warp 1 = MMA issuer
+// (owns the TMEM allocation), warps 2-5 = epilogue (one thread per accumulator row).  Two CTAs fit an SM at
+// BN = 64, so one tile's epilogue overlaps the other's main loop; these contractions have K = 192..768 only and
+// are bound by HBM and the epilogue, not by the tensor pipe.
+#include "gemm_tc.cuh"
+
+#include <cudaTypedefs.h>
+
+#include "common.cuh"
+#include "device.h"
+#include "tc_common.cuh"
+
+namespace tabattn {
+namespace gemm {
+
+namespace {
+
+using namespace tc;
+
+constexpr int BM = 128, BK = 64;
+constexpr int kThreads = 192;
+constexpr int A_BYTES = BM * BK * 2;   // 16 KB, either layout
+
+struct KParams {
+  int M, N, K;
+  int kb_total, kb_per_slab, slabs;
+  float alpha, beta;
+  const float* row_scale;
+  int act, aux_mode;
+  float* partial;
+  int split_cols;
+  int a_batched, b_batched;   // 0: operand shared by all batches (TMA batch coordinate 0)
+  int a_split_k;              // > 0: A is three tensors of this many columns
+  int dual_out;
+};
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(
+                   reinterpret_cast<uint64_t>(m)),
+               "r"(src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+
+__device__ __forceinline__ float gelu_f(float x) { return 0.5f * x * (1.f + erff(x * 0.70710678118654752f)); }
+__device__ __forceinline__ float gelu_grad_f(float x) {
+  return 0.5f * (1.f + erff(x * 0.70710678118654752f)) + x * 0.3989422804014327f * __expf(-0.5f * x * x);
+}
+
+template <int BN>
+struct Cfg {
+  static constexpr int ST = BN == 64 ? 3 : 4;   // (two CTAs per SM at BN = 64)
+  static constexpr int B_BYTES = BN * BK * 2;
+  static constexpr int STAGE = A_BYTES + B_BYTES;
+  static constexpr int STAGING = (BN / 64) * (BM * 128);
+  static constexpr int SMEM = ST * STAGE + STAGING + 1024;
+};
+
+template <int BN, int A_MN, int B_MN>
+__global__ void __launch_bounds__(kThreads)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA2,
+               const __grid_constant__ CUtensorMap mapA3, const __grid_constant__ CUtensorMap mapB,
+               const __grid_constant__ CUtensorMap mapAux, const __grid_constant__ CUtensorMap mapC0,
+               const __grid_constant__ CUtensorMap mapC1, const __grid_constant__ CUtensorMap mapC2,
+               const __grid_constant__ KParams p) {
+  using C = Cfg<BN>;
+  constexpr int ST = C::ST;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sA = sbase, sB = sA + ST * A_BYTES, sOut = sB + ST * C::B_BYTES;
+  __shared__ uint64_t bar_full[ST], bar_empty[ST], bar_acc, bar_aux;
+  __shared__ uint32_t tmem_slot;
+
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+  const int n0 = blockIdx.x * BN, m0 = blockIdx.y * BM;
+  const bool splitk = p.partial != nullptr;   // fp32 partial tiles instead of the bf16 output
+  const int bz = splitk ? 0 : blockIdx.z, slab = splitk ? blockIdx.z : 0;
+  const int kb0 = slab * p.kb_per_slab, kb1 = min(p.kb_total, kb0 + p.kb_per_slab);
+
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), BN);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < ST; ++i) {
+      mbar_init(smem_u32(&bar_full[i]), 1);
+      mbar_init(smem_u32(&bar_empty[i]), 1);
+    }
+    mbar_init(smem_u32(&bar_acc), 1);
+    mbar_init(smem_u32(&bar_aux), 1);
+    fence_barrier_init();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      tma_prefetch_desc(&mapA);
+      tma_prefetch_desc(&mapB);
+      const int ba = p.a_batched ? bz : 0, bb = p.b_batched ? bz : 0;
+      if (p.aux_mode != AUX_NONE) {
+        // the tile of the auxiliary operand lands in the staging tile the epilogue later overwrites in place
+        mbar_arrive_expect_tx(smem_u32(&bar_aux), C::STAGING);
+#pragma unroll
+        for (int h = 0; h < BN / 64; ++h) tma_load_3d(sOut + h * (BM * 128), &mapAux, smem_u32(&bar_aux), n0 + 64 * h, m0, bz);
+      }
+      uint32_t t = 0;
+      for (int kb = kb0; kb < kb1; ++kb, ++t) {
+        const uint32_t st = t % ST, full = smem_u32(&bar_full[st]);
+        mbar_wait<true>(smem_u32(&bar_empty[st]), ((t / ST) & 1) ^ 1);
+        mbar_arrive_expect_tx(full, C::STAGE);
+        const uint32_t a = sA + st * A_BYTES, b = sB + st * C::B_BYTES;
+        if (A_MN) {
+          tma_load_3d(a, &mapA, full, m0, kb * BK, ba);
+          tma_load_3d(a + 64 * 128, &mapA, full, m0 + 64, kb * BK, ba);
+        } else if (p.a_split_k > 0) {
+          const int seg = (kb * BK) / p.a_split_k, kin = kb * BK - seg * p.a_split_k;
+          tma_load_3d(a, seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3), full, kin, m0, ba);
+        } else {
+          tma_load_3d(a, &mapA, full, kb * BK, m0, ba);
+        }
+        if (B_MN) {
+#pragma unroll
+          for (int h = 0; h < BN / 64; ++h) tma_load_3d(b + h * (64 * 128), &mapB, full, n0 + 64 * h, kb * BK, bb);
+        } else {
+          tma_load_3d(b, &mapB, full, kb * BK, n0, bb);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    constexpr uint32_t idesc = make_idesc_bf16(BM, BN, A_MN != 0, B_MN != 0);
+    // K-major: rows of 128 bytes, 8-row groups 1024 bytes apart, 32 bytes per k-step.
+    // MN-major: [64 k-rows][128 bytes] atoms of 64 M/N elements, 8192 bytes apart; 16 k-rows = 2048 bytes per k-step.
+    const uint64_t dA = A_MN ? make_smem_desc<128>(sA, 64 * 128, 1024) : make_smem_desc<128>(sA, 16, 1024);
+    const uint64_t dB = B_MN ? make_smem_desc<128>(sB, 64 * 128, 1024) : make_smem_desc<128>(sB, 16, 1024);
+    uint32_t t = 0;
+    for (int kb = kb0; kb < kb1; ++kb, ++t) {
+      const uint32_t st = t % ST;
+      mbar_wait(smem_u32(&bar_full[st]), (t / ST) & 1);
+      tc_fence_after();
+      const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
+#pragma unroll
+      for (int kk = 0; kk < BK / 16; ++kk)
+        mma_ss_e(tmem, a + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc, (t > 0 || kk > 0) ? 1u : 0u);
+      tc_commit_e(smem_u32(&bar_empty[st]));
+    }
+    tc_commit_e(smem_u32(&bar_acc));
+  } else {
+    // ------------------------------------------------------------------------------ epilogue
+    const int q = warp & 3, r = 32 * q + lane;
+    const int m = m0 + r;
+    const uint32_t tacc = tmem + ((uint32_t)(32 * q) << 16);
+    float rs = p.alpha;
+    if (p.row_scale && m < p.M) rs *= __ldg(p.row_scale + (size_t)bz * p.M + m);
+    mbar_wait(smem_u32(&bar_acc), 0);
+    tc_fence_after();
+    if (p.aux_mode != AUX_NONE) mbar_wait(smem_u32(&bar_aux), 0);
+    const bool has_k = kb1 > kb0;
+    const int passes = p.dual_out ? 2 : 1;
+    for (int pass = 0; pass < passes; ++pass) {
+      // dual output: pass 0 stores the value before the activation (C0), pass 1 the value after it (C1)
+      const bool do_act = p.act == ACT_GELU && (!p.dual_out || pass == 1);
+#pragma unroll 1
+      for (int c = 0; c < BN / 32; ++c) {
+        uint32_t v[32];
+        tmem_ld32(tacc + 32 * c, v);
+        tmem_wait_ld();
+        if (!has_k) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = 0u;
+        }
+        if (splitk) {
+          if (m < p.M) {
+            float* dst = p.partial + ((size_t)slab * p.M + m) * p.N + n0 + 32 * c;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              if (n0 + 32 * c + 4 * j < p.N)
+                *reinterpret_cast<float4*>(dst + 4 * j) =
+                    make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+          }
+          continue;
+        }
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          const int col = 32 * c + 8 * ch;                       // first of 8 columns inside the tile
+          const uint32_t off = sOut + (uint32_t)(col >> 6) * (BM * 128) + (uint32_t)r * 128 +
+                               (uint32_t)((((col & 63) >> 3) ^ (r & 7)) << 4);
+          float f[8], a[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[8 * ch + e]) * rs;
+          if (p.aux_mode != AUX_NONE) {
+            const uint4 u = lds_v4(off);
+            unpack8(u, a);
+          }
+          if (p.aux_mode == AUX_ADD) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) f[e] = fmaf(p.beta, a[e], f[e]);
+          }
+          if (do_act) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) f[e] = gelu_f(f[e]);
+          }
+          if (p.aux_mode == AUX_GELU_GRAD) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) f[e] *= gelu_grad_f(a[e]);
+          }
+          const uint4 o = pack8(f);
+          sts_v4(off, o.x, o.y, o.z, o.w);
+        }
+      }
+      if (splitk) break;
+      fence_proxy_async_smem();
+      named_bar_sync(1, 128);
+      if (warp == 2 && lane == 0) {
+#pragma unroll
+        for (int h = 0; h < BN / 64; ++h) {
+          const int col = n0 + 64 * h;
+          if (col >= p.N) continue;
+          int t = p.split_cols > 0 ? col / p.split_cols : 0;
+          const int cin = col - t * p.split_cols;
+          if (p.dual_out) t = pass;
+          const CUtensorMap* mc = t == 0 ? &mapC0 : (t == 1 ? &mapC1 : &mapC2);
+          tma_store_3d(mc, sOut + h * (BM * 128), cin, m0, bz);
+        }
+        bulk_commit();
+        bulk_wait<0>();
+      }
+      // (dual output: the staging tile is rewritten by the next pass only after the store has read it)
+      if (passes > 1) named_bar_sync(1, 128);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem, BN);
+}
+
+__global__ void reduce_slabs_kernel(const float* __restrict__ partial, int slabs, long long mn, float scale,
+                                    void* __restrict__ out, int out_f32) {
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (i >= mn) return;
+  float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int s = 0; s < slabs; ++s) {
+    const float4 v = *reinterpret_cast<const float4*>(partial + (long long)s * mn + i);
+    a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+  }
+  a.x *= scale; a.y *= scale; a.z *= scale; a.w *= scale;
+  if (out_f32) {
+    *reinterpret_cast<float4*>(static_cast<float*>(out) + i) = a;
+  } else {
+    uint2 o;
+    o.x = pack_bf16(a.x, a.y);
+    o.y = pack_bf16(a.z, a.w);
+    *reinterpret_cast<uint2*>(static_cast<uint16_t*>(out) + i) = o;
+  }
+}
+
+PFN_cuTensorMapEncodeTiled_v12000 encode_fn() {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = []() -> PFN_cuTensorMapEncodeTiled_v12000 {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+  }();
+  return fn;
+}
+
+// bf16 matrix [rows][inner] (pitch ld elements) x batch -> 3-D map, box (64 inner, box_rows, 1), 128-byte swizzle
+bool make_map(CUtensorMap* m, const void* ptr, long long inner, long long rows, long long ld, int batch,
+              long long batch_stride, int box_rows) {
+  auto fn = encode_fn();
+  if (!fn || !ptr) return false;
+  const bool shared = batch_stride == 0 || batch <= 1;
+  cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)(shared ? 1 : batch)};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * 2, (cuuint64_t)(shared ? rows * ld : batch_stride) * 2};
+  cuuint32_t box[3] = {64, (cuuint32_t)box_rows, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int BN, int A_MN, int B_MN>
+cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
+  const DeviceInfo* di = current_device();
+  if (!di) return cudaErrorInvalidDevice;
+  CUtensorMap ma, ma2, ma3, mb, maux, mc[3];
+  // A: K-major -> stored [M][K]: inner K, box rows 128; MN-major -> stored [K][M]: inner M, box 64 k-rows
+  bool ok = p.A.mn_major ? make_map(&ma, p.A.ptr, p.M, p.K, p.A.ld, p.batch, p.A.batch_stride, 64)
+                         : make_map(&ma, p.A.ptr, p.K, p.M, p.A.ld, p.batch, p.A.batch_stride, BM);
+  ma2 = ma; ma3 = ma;
+  if (p.a_split_k > 0) {
+    ok = ok && !p.A.mn_major && make_map(&ma, p.A.ptr, p.a_split_k, p.M, p.A.ld, p.batch, p.A.batch_stride, BM) &&
+         make_map(&ma2, p.A2, p.a_split_k, p.M, p.A.ld, p.batch, p.A.batch_stride, BM) &&
+         make_map(&ma3, p.A3, p.a_split_k, p.M, p.A.ld, p.batch, p.A.batch_stride, BM);
+  }
+  ok = ok && (p.B.mn_major ? make_map(&mb, p.B.ptr, p.N, p.K, p.B.ld, p.batch, p.B.batch_stride, 64)
+                           : make_map(&mb, p.B.ptr, p.K, p.N, p.B.ld, p.batch, p.B.batch_stride, BN));
+  const int nout = p.partial ? 0 : (p.dual_out ? 2 : (p.split_cols > 0 ? (p.N + p.split_cols - 1) / p.split_cols : 1));
+  const long long out_cols = p.split_cols > 0 ? p.split_cols : p.N;
+  for (int t = 0; t < 3; ++t) {
+    if (t < nout) ok = ok && make_map(&mc[t], p.C[t], out_cols, p.M, p.ldc, p.batch, p.c_batch_stride, BM);
+    else mc[t] = t > 0 && nout > 0 ? mc[0] : ma;
+  }
+  if (p.aux_mode != AUX_NONE) ok = ok && make_map(&maux, p.aux, p.N, p.M, p.ld_aux, p.batch, p.aux_batch_stride, BM);
+  else maux = ma;
+  if (!ok) return cudaErrorInvalidValue;
+  auto kern = gemm_tc_kernel<BN, A_MN, B_MN>;
+  static SmemAttr attr;
+  cudaError_t e = attr.ensure(kern, Cfg<BN>::SMEM, di->ordinal);
+  if (e != cudaSuccess) return e;
+  dim3 grid((p.N + BN - 1) / BN, (p.M + BM - 1) / BM, p.partial ? kp.slabs : p.batch);
+  kern<<<grid, kThreads, Cfg<BN>::SMEM, stream>>>(ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
+  count_launch();
+  return cudaGetLastError();
+}
+
+template <int BN>
+cudaError_t launch_bn(const Problem& p, const KParams& kp, cudaStream_t stream) {
+  if (!p.A.mn_major && !p.B.mn_major) return launch_t<BN, 0, 0>(p, kp, stream);
+  if (!p.A.mn_major && p.B.mn_major) return launch_t<BN, 0, 1>(p, kp, stream);
+  if (p.A.mn_major && p.B.mn_major) return launch_t<BN, 1, 1>(p, kp, stream);
+  return cudaErrorInvalidValue;   // (A MN-major with B K-major is not needed by any caller)
+}
+
+}  // namespace
+
+int slabs_for(long long K, int tiles, int num_sms) {
+  const long long kb_total = (K + BK - 1) / BK;
+  long long want = (2LL * num_sms + tiles - 1) / tiles;
+  want = want < 1 ? 1 : (want > 128 ? 128 : want);
+  if (want > kb_total) want = kb_total;
+  const long long per = (kb_total + want - 1) / want;
+  return (int)((kb_total + per - 1) / per);
+}
+
+cudaError_t launch(const Problem& p, cudaStream_t stream) {
+  if (p.M < 1 || p.N < 1 || p.K < 1 || p.batch < 1) return cudaErrorInvalidValue;
+  // TMA: row pitches are multiples of 16 bytes; the extents themselves are free (out-of-range box parts read 0)
+  if ((p.A.ld & 7) || (p.B.ld & 7) || (!p.partial && (p.ldc & 7)) || (p.aux_mode != AUX_NONE && (p.ld_aux & 7)))
+    return cudaErrorInvalidValue;
+  if (p.slabs > 1 && !p.partial) return cudaErrorInvalidValue;
+  if (p.partial && (p.batch != 1 || (p.N & 3))) return cudaErrorInvalidValue;
+  if (p.split_cols > 0 && (p.split_cols % 64 != 0)) return cudaErrorInvalidValue;
+  KParams kp{};
+  kp.M = p.M; kp.N = p.N; kp.K = p.K;
+  kp.kb_total = (p.K + BK - 1) / BK;
+  const int want = p.slabs > 1 ? p.slabs : 1;
+  kp.kb_per_slab = (kp.kb_total + want - 1) / want;
+  kp.slabs = (kp.kb_total + kp.kb_per_slab - 1) / kp.kb_per_slab;
+  if (kp.slabs != want) return cudaErrorInvalidValue;   // (callers size slabs with gemm::slabs_for)
+  kp.alpha = p.alpha; kp.beta = p.beta; kp.row_scale = p.row_scale; kp.act = p.act; kp.aux_mode = p.aux_mode;
+  kp.partial = p.partial; kp.split_cols = p.split_cols;
+  kp.a_batched = p.A.batch_stride != 0; kp.b_batched = p.B.batch_stride != 0;
+  kp.a_split_k = p.a_split_k; kp.dual_out = p.dual_out;
+  if (p.a_split_k > 0 && (p.a_split_k % 64 != 0 || p.K != 3 * p.a_split_k || !p.A2 || !p.A3)) return cudaErrorInvalidValue;
+  if (p.dual_out && (p.split_cols > 0 || p.partial)) return cudaErrorInvalidValue;
+  // 128-wide tiles when N allows it (fewer re-reads of A), else 64; split outputs need 64-column granularity
+  const bool bn128 = (p.N % 128 == 0) && (p.split_cols == 0 || p.split_cols % 128 == 0);
+  return bn128 ? launch_bn<128>(p, kp, stream) : launch_bn<64>(p, kp, stream);
+}
+
+cudaError_t launch_reduce_slabs(const float* partial, int slabs, long long mn, float scale, void* out, bool out_f32,
+                                cudaStream_t stream) {
+  if (mn & 3) return cudaErrorInvalidValue;
+  const int threads = 256;
+  const long long blocks = (mn / 4 + threads - 1) / threads;
+  reduce_slabs_kernel<<<(unsigned)blocks, threads, 0, stream>>>(partial, slabs, mn, scale, out, out_f32 ? 1 : 0);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace gemm
+}  // namespace tabattn

@@ -32,4 +32,26 @@ cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const 
                             cudaStream_t stream);
 size_t item_bwd_workspace_bytes(const Shape& s);
 
+// ---- sub-blocks around the attention kernels (block_ops.cu) ------------------------
+size_t block_ws_bytes(long long cells, int e, int hidden_or_zero, int num_sms);
+cudaError_t launch_mlp_fwd(long long cells, int e, int hidden, float alpha, float eps, const void* x, const void* g,
+                           const void* W1, const void* W2, void* y, void* h, float* rstd, void* u, void* a,
+                           cudaStream_t stream);
+cudaError_t launch_mlp_bwd(long long cells, int e, int hidden, float alpha, const void* x, const void* g,
+                           const void* W1, const void* W2, const void* h, const float* rstd, const void* u,
+                           const void* a, const void* dy, void* dx, float* dg, float* dW1, float* dW2, void* ws,
+                           size_t ws_bytes, cudaStream_t stream);
+cudaError_t launch_attn_block_fwd(const Shape& s, int axis, float alpha, float eps, const void* x, const void* g,
+                                  const void* Wqkv, const void* Wo, void* y, void* h, float* rstd, void* q, void* k,
+                                  void* v, void* o, float* lse, void* ws, cudaStream_t stream);
+size_t attn_block_bwd_ws_bytes(const Shape& s, int axis, int num_sms);
+cudaError_t launch_attn_block_bwd(const Shape& s, int axis, float alpha, const void* x, const void* g,
+                                  const void* Wqkv, const void* Wo, const void* h, const float* rstd, const void* q,
+                                  const void* k, const void* v, const void* o, const float* lse, const void* dy,
+                                  void* dx, float* dg, float* dWqkv, float* dWo, void* ws, size_t ws_bytes,
+                                  cudaStream_t stream);
+size_t newton_schulz_ws_bytes(int nb, int m, int n);
+cudaError_t launch_newton_schulz(int nb, int m, int n, const void* G, void* X, int steps, float ca, float cb, float cc,
+                                 float eps, void* ws, cudaStream_t stream);
+
 }  // namespace tabattn
