@@ -362,6 +362,106 @@ def time_workload(torch, dist, tab, wl, steps, warmup, min_region_s, world, rank
             "call_ms": call_ms, "launches": int(launches), "clocks": clocks}
 
 
+# ---- the rows SURVEY.md §8(f) marks "next": evaluation path, sub-blocks, Newton-Schulz ------------------------------
+def _timeit(torch, stream, fn, iters, warmup=3):
+    for _ in range(warmup):
+        fn()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record(stream)
+    for _ in range(iters):
+        fn()
+    b.record(stream)
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / iters
+
+
+def time_next_rows(torch, tab, dev, peaks, iters=20):
+    """Device times of the §8(f) rows on seeded synthetic inputs resident in HBM (inputs larger than L2 except
+    Newton-Schulz, which is launch-bound and says so).  Algorithmic work per DESIGN.md §5.2."""
+    out = {}
+    stream = torch.cuda.current_stream()
+    g = torch.Generator(device=dev)
+    g.manual_seed(1234)
+    bf = torch.bfloat16
+
+    def rnd(*shape, scale=1.0):
+        return (torch.randn(*shape, generator=g, device=dev, dtype=torch.float32) * scale).to(bf)
+
+    # (f)-2 evaluation path: PAPER.md:L65 table (24 thinking + 800 train + 200 test rows, 100 features + target),
+    # record width (256, 4 heads); five folds batched.  Whole block (all rows) and last block (test rows only).
+    B, R, C, H, dh, n = 5, 1024, 101, 4, 64, 824
+    d = H * dh
+    Q, K, V = (rnd(B, R, C, H, dh) for _ in range(3))
+    O = torch.empty_like(Q)
+    nt = torch.full((B,), n, dtype=torch.int32, device=dev)
+    ev = {}
+    for name, r0, r1 in (("all_rows", 0, R), ("test_rows", n, R)):
+        tf = _timeit(torch, stream, lambda: tab.tabattn_feature_fwd_infer(Q, K, V, r0, r1, O=O), iters)
+        ti = _timeit(torch, stream, lambda: tab.tabattn_item_fwd_infer(Q, K, V, nt, r0, r1, O=O), iters)
+        rows = r1 - r0
+        fb = B * rows * C * 8 * d                       # Q, K, V in, O out (no LSE)
+        ifl = 4 * B * C * rows * n * d
+        ib = B * C * (2 * rows + 2 * n) * 2 * d
+        ev[name] = {"feature_fwd_infer": {"ms": tf, "GB/s": fb / tf / 1e6, "frac_hbm": fb / tf / 1e6 / peaks["hbm_gbs"]},
+                    "item_fwd_infer": {"ms": ti, "TFLOP/s": ifl / ti / 1e9, "GB/s": ib / ti / 1e6,
+                                       "frac_tensor_burst": ifl / ti / 1e9 / peaks["bf16_tflops"]}}
+    out["eval_1000x100"] = {"shape": {"B": B, "R": R, "C": C, "H": H, "dh": dh, "n_train": n}, **ev}
+    del Q, K, V, O
+    torch.cuda.empty_cache()
+
+    # (f)-1 / (f)-3 sub-blocks on the long_item table shape (cells = 8 x 4096 x 21, e = 256, hidden = 768)
+    cfg = get_config("long_item")
+    B, R, C, H, dh = cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh
+    e, hid, cells, alpha = H * dh, 768, cfg.B * cfg.R * cfg.C, 0.95
+    x, dy = rnd(B, R, C, e), rnd(B, R, C, e)
+    gain = (1 + 0.1 * torch.randn(e, generator=g, device=dev)).to(bf)
+    Wqkv, Wo = rnd(3 * e, e, scale=e ** -0.5), rnd(e, e, scale=e ** -0.5)
+    W1, W2 = rnd(hid, e, scale=e ** -0.5), rnd(e, hid, scale=hid ** -0.5)
+    nt = torch.full((B,), cfg.n_train, dtype=torch.int32, device=dev)
+    blocks = {}
+    for axis, nm in ((0, "feature"), (1, "item")):
+        y, sv = tab.tabattn_attn_block_fwd(axis, x, gain, Wqkv, Wo, H, nt, None, alpha)
+        wsf = torch.empty(int(tab.lib().tabattn_attn_block_workspace_bytes(
+            __import__("ctypes").byref(tab.make_shape(x.view(B, R, C, H, dh), nt)[0]), axis, 1)), dtype=torch.uint8, device=dev)
+        tfw = _timeit(torch, stream, lambda: tab.tabattn_attn_block_fwd(axis, x, gain, Wqkv, Wo, H, nt, None, alpha,
+                                                                        saved=sv, y=y), iters)
+        tbw = _timeit(torch, stream, lambda: tab.tabattn_attn_block_bwd(axis, x, gain, Wqkv, Wo, H, sv, dy, nt, None,
+                                                                        alpha, ws=wsf), iters)
+        proj_f, proj_b = 8 * cells * e * e, 16 * cells * e * e       # QKV + out projections: 4 e^2 MACs / cell fwd
+        att_f = 4 * cells * (C if axis == 0 else cfg.n_train) * e
+        att_b = 10 * cells * (C if axis == 0 else cfg.n_train) * e
+        blocks["attn_block_" + nm] = {"fwd_ms": tfw, "bwd_ms": tbw,
+                                      "fwd_TFLOP/s": (proj_f + att_f) / tfw / 1e9,
+                                      "bwd_TFLOP/s": (proj_b + att_b) / tbw / 1e9}
+        del sv, wsf, y
+    y, sv = tab.tabattn_mlp_fwd(x, gain, W1, W2, alpha)
+    wsm = torch.empty(int(tab.lib().tabattn_mlp_workspace_bytes(cells, e, hid)), dtype=torch.uint8, device=dev)
+    tfw = _timeit(torch, stream, lambda: tab.tabattn_mlp_fwd(x, gain, W1, W2, alpha, saved=sv, y=y), iters)
+    tbw = _timeit(torch, stream, lambda: tab.tabattn_mlp_bwd(x, gain, W1, W2, sv, dy, alpha, ws=wsm), iters)
+    ff, fbw = 4 * cells * e * hid, 8 * cells * e * hid
+    bytes_f, bytes_b = cells * (4 * e + 2 * hid), cells * (6 * e + 2 * hid)   # x, y, saved u | x, dy, u, dx
+    blocks["mlp_block"] = {"fwd_ms": tfw, "bwd_ms": tbw, "fwd_TFLOP/s": ff / tfw / 1e9, "bwd_TFLOP/s": fbw / tbw / 1e9,
+                           "fwd_frac_tensor_burst": ff / tfw / 1e9 / peaks["bf16_tflops"],
+                           "bwd_frac_tensor_burst": fbw / tbw / 1e9 / peaks["bf16_tflops"],
+                           "fwd_frac_hbm": bytes_f / tfw / 1e6 / peaks["hbm_gbs"],
+                           "bwd_frac_hbm": bytes_b / tbw / 1e6 / peaks["hbm_gbs"]}
+    out["blocks_long_item_shape"] = {"cells": cells, "e": e, "hidden": hid, **blocks}
+    del x, dy, y, sv, wsm
+    torch.cuda.empty_cache()
+
+    # (f)-4 batched Newton-Schulz over the QKV matrices of the record model: 5 blocks x 2 attentions x 3 (PAPER.md:L95)
+    nb, m = 30, 256
+    G = rnd(nb, m, m, scale=0.02)
+    X = torch.empty_like(G)
+    wsn = torch.empty(int(tab.lib().tabattn_newton_schulz_workspace_bytes(nb, m, m)), dtype=torch.uint8, device=dev)
+    tns = _timeit(torch, stream, lambda: tab.tabattn_newton_schulz(G, 5, X=X, ws=wsn), iters)
+    fl = nb * 5 * 6 * m ** 3
+    out["newton_schulz"] = {"nb": nb, "m": m, "n": m, "steps": 5, "ms": tns, "TFLOP/s": fl / tns / 1e9,
+                            "launches": 16, "note": "30 matrices of 256x256 (3.9 MB): L2-resident and launch-bound"}
+    return out
+
+
 def static_traffic(cfg_name, call):
     """DRAM bytes (read + write) of one C-ABI call from the committed ncu --set full capture
     (profiles/r02_traffic.csv; falls back to round 1's).  A static capture, not measured in this run."""
@@ -452,6 +552,10 @@ def run_ours(args):
             del w2
             torch.cuda.empty_cache()
 
+    next_rows = None
+    if world == 1 and not args.no_extra:
+        next_rows = time_next_rows(torch, tab, dev, peaks)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -503,6 +607,7 @@ def run_ours(args):
                              % ((work["feature_fwd_bytes"] + work["item_fwd_bytes"]) / 1e6)},
             "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
             "clocks": m["clocks"], "calls": call_table(call_ms, work, peaks, region_s), "configs": others,
+            "next_rows": next_rows,
             "peaks": {k: peaks[k] for k in ("hbm_gbs", "bf16_tflops", "bf16_tflops_sustained", "source")},
             "context": {"paper_l40s_baseline_min": 74.32, "paper_l40s_record_min": 0.92,
                         "note": "full-pretraining wallclock on 1x L40S (PAPER.md:L43, L51); context, not the target"}}

@@ -1,7 +1,7 @@
-// tcgen05 GEMM core (gemm_tc.cuh): one 128 x BN output tile per CTA, a 4-stage TMA ring over 64-wide k-blocks,
+// tcgen05 GEMM core (gemm_tc.cuh): one 128 x BN output tile per CTA, a 2-3 stage TMA ring over 64-wide k-blocks,
 // fp32 accumulator in TMEM, fused epilogue, TMA store.  Warp 0 = TMA producer (one lane), warp 1 = MMA issuer
-// (owns the TMEM allocation), warps 2-5 = epilogue (one thread per accumulator row).  Two CTAs fit an SM at
-// BN = 64, so one tile's epilogue overlaps the other's main loop; these contractions have K = 192..768 only and
+// (owns the TMEM allocation), warps 2-9 = epilogue (one thread per accumulator row and column half).  Two CTAs fit an SM,
+// so one tile's epilogue overlaps the other's main loop; these contractions have K = 192..768 only and
 // are bound by HBM and the epilogue, not by the tensor pipe.
 #include "gemm_tc.cuh"
 
@@ -19,7 +19,8 @@ namespace {
 using namespace tc;
 
 constexpr int BM = 128, BK = 64;
-constexpr int kThreads = 192;
+constexpr int kEpiWarps = 8;                     // two per TMEM lane quadrant, each half of the tile's columns
+constexpr int kThreads = (2 + kEpiWarps) * 32;
 constexpr int A_BYTES = BM * BK * 2;   // 16 KB, either layout
 
 struct KParams {
@@ -48,14 +49,32 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src,
                : "memory");
 }
 
-__device__ __forceinline__ float gelu_f(float x) { return 0.5f * x * (1.f + erff(x * 0.70710678118654752f)); }
+// erf by Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7, far below the bf16 step of the outputs): one reciprocal, one
+// ex2 and five FMAs instead of erff's ~30 instructions -- the epilogue of the MLP GEMMs is bound by this arithmetic.
+// Returns erf(x / sqrt 2) and leaves exp(-x^2 / 2) in `ex` (the Gaussian factor of gelu').
+__device__ __forceinline__ float erf_half(float x, float& ex) {
+  const float z = fabsf(x) * 0.70710678118654752f;
+  const float t = __frcp_rn(fmaf(0.3275911f, z, 1.f));
+  ex = fast_exp2(-z * z * kLog2e);
+  float p = fmaf(t, 1.061405429f, -1.453152027f);
+  p = fmaf(p, t, 1.421413741f);
+  p = fmaf(p, t, -0.284496736f);
+  p = fmaf(p, t, 0.254829592f);
+  return copysignf(fmaf(-p * t, ex, 1.f), x);
+}
+__device__ __forceinline__ float gelu_f(float x) {
+  float ex;
+  return 0.5f * x * (1.f + erf_half(x, ex));
+}
 __device__ __forceinline__ float gelu_grad_f(float x) {
-  return 0.5f * (1.f + erff(x * 0.70710678118654752f)) + x * 0.3989422804014327f * __expf(-0.5f * x * x);
+  float ex;
+  const float er = erf_half(x, ex);
+  return fmaf(x * 0.3989422804014327f, ex, 0.5f * (1.f + er));
 }
 
 template <int BN>
 struct Cfg {
-  static constexpr int ST = BN == 64 ? 3 : 4;   // (two CTAs per SM at BN = 64)
+  static constexpr int ST = BN == 64 ? 3 : 2;   // two CTAs per SM: one tile's epilogue overlaps the other's main loop
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE = A_BYTES + B_BYTES;
   static constexpr int STAGING = (BN / 64) * (BM * 128);
@@ -63,7 +82,7 @@ struct Cfg {
 };
 
 template <int BN, int A_MN, int B_MN>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 2)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA2,
                const __grid_constant__ CUtensorMap mapA3, const __grid_constant__ CUtensorMap mapB,
                const __grid_constant__ CUtensorMap mapAux, const __grid_constant__ CUtensorMap mapC0,
@@ -153,6 +172,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   } else {
     // ------------------------------------------------------------------------------ epilogue
     const int q = warp & 3, r = 32 * q + lane;
+    const int c_lo = ((warp - 2) >> 2) * (BN / 64), c_hi = c_lo + BN / 64;   // this warp's 32-column groups
     const int m = m0 + r;
     const uint32_t tacc = tmem + ((uint32_t)(32 * q) << 16);
     float rs = p.alpha;
@@ -166,7 +186,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       // dual output: pass 0 stores the value before the activation (C0), pass 1 the value after it (C1)
       const bool do_act = p.act == ACT_GELU && (!p.dual_out || pass == 1);
 #pragma unroll 1
-      for (int c = 0; c < BN / 32; ++c) {
+      for (int c = c_lo; c < c_hi; ++c) {
         uint32_t v[32];
         tmem_ld32(tacc + 32 * c, v);
         tmem_wait_ld();
@@ -216,7 +236,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       }
       if (splitk) break;
       fence_proxy_async_smem();
-      named_bar_sync(1, 128);
+      named_bar_sync(1, kEpiWarps * 32);
       if (warp == 2 && lane == 0) {
 #pragma unroll
         for (int h = 0; h < BN / 64; ++h) {
@@ -232,7 +252,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         bulk_wait<0>();
       }
       // (dual output: the staging tile is rewritten by the next pass only after the store has read it)
-      if (passes > 1) named_bar_sync(1, 128);
+      if (passes > 1) named_bar_sync(1, kEpiWarps * 32);
     }
   }
   tc_fence_before();

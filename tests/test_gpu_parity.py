@@ -227,3 +227,59 @@ def test_layer_is_graph_capturable():
         torch.cuda.synchronize()
         for got, w in zip(outs, want):
             assert torch.equal(got.view(torch.int16), w.view(torch.int16)), "replay %d" % rep
+
+
+# ---- out-of-bounds writes: guard bands (compute-sanitizer is closed on this pool, profiles/r02_sanitizer.md) --------
+GUARD = 4096   # bytes of sentinel before and after every output buffer
+
+
+def _guarded(torch, nbytes):
+    """A uint8 buffer [guard | payload | guard] filled with 0xA5; returns (whole, payload view)."""
+    whole = torch.full((nbytes + 2 * GUARD,), 0xA5, dtype=torch.uint8, device="cuda")
+    return whole, whole[GUARD:GUARD + nbytes]
+
+
+def _guards_intact(whole):
+    return bool((whole[:GUARD] == 0xA5).all()) and bool((whole[-GUARD:] == 0xA5).all())
+
+
+@pytest.mark.parametrize("axis", ["feature", "item"])
+@pytest.mark.parametrize("shape", [("tiny", 2, 64, 6, 2, 16, 48), ("edges", 1, 257, 4, 2, 32, 129),
+                                   ("odd64", 2, 131, 23, 2, 64, 77), ("masked", 3, 75, 19, 3, 32, 50)],
+                         ids=lambda s: s[0])
+def test_no_write_outside_the_output_buffers(shape, axis):
+    """Every output and the workspace sit between sentinel bands; the bands must survive fwd + bwd (a write past
+    the tensor -- a tile tail, a clipped TMA box, a zero-fill loop -- would land in them)."""
+    import torch
+    import paper_2606_03681_b200 as tab
+    gu = _gu()
+    name, B, R, C, H, dh, n = shape
+    cfg = TabShape(name, 91, B=B, R=R, C=C, H=H, dh=dh, n_train=n, mask="subset" if name == "masked" else "none",
+                   valid_features=(3, C - 1) if name == "masked" else None)
+    n_train, col_valid = draw_structure(cfg)
+    inp = {k: gu.to_dev(v) for k, v in make_call_inputs(cfg, axis).items()}
+    cv = torch.from_numpy(np.ascontiguousarray(col_valid, dtype=np.uint8)).cuda() if col_valid is not None else None
+    nt = torch.from_numpy(n_train).cuda()
+    cells_b = B * R * C * H * dh * 2
+    lse_shape = (B, R, H, C) if axis == "feature" else (B, C, H, R)
+    bufs = {k: _guarded(torch, cells_b) for k in ("O", "dQ", "dK", "dV")}
+    bufs["LSE"] = _guarded(torch, B * R * C * H * 4)
+    shp, _keep = tab.make_shape(inp["Q"], nt, cv)
+    need = max(tab.workspace_bytes(shp, op) for op in range(4))
+    bufs["ws"] = _guarded(torch, max(need, 16))
+    t5 = lambda k: bufs[k][1].view(torch.bfloat16).view(B, R, C, H, dh)
+    LSE = bufs["LSE"][1].view(torch.float32).view(lse_shape)
+    ws = bufs["ws"][1]
+    if axis == "feature":
+        tab.tabattn_feature_fwd(inp["Q"], inp["K"], inp["V"], cv, O=t5("O"), LSE=LSE, ws=ws)
+        tab.tabattn_feature_bwd(inp["Q"], inp["K"], inp["V"], t5("O"), inp["dO"], LSE, cv, dQ=t5("dQ"), dK=t5("dK"),
+                                dV=t5("dV"), ws=ws)
+    else:
+        tab.tabattn_item_fwd(inp["Q"], inp["K"], inp["V"], nt, cv, O=t5("O"), LSE=LSE, ws=ws)
+        tab.tabattn_item_bwd(inp["Q"], inp["K"], inp["V"], t5("O"), inp["dO"], LSE, nt, cv, dQ=t5("dQ"), dK=t5("dK"),
+                             dV=t5("dV"), ws=ws)
+    torch.cuda.synchronize()
+    for k, (whole, payload) in bufs.items():
+        assert _guards_intact(whole), "%s/%s: a kernel wrote outside %s" % (name, axis, k)
+        if k in ("O", "dQ", "dK", "dV"):
+            assert not bool((payload == 0xA5).all()), "%s was not written" % k
