@@ -497,6 +497,11 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.only_next_rows:
+        # profiling helper: only the SURVEY.md §8(f) rows, few iterations (ncu captures of the GEMM / norm kernels)
+        print(json.dumps({"next_rows": time_next_rows(torch, tab, dev, peaks, iters=args.steps)}))
+        return 0
+
     # ---- headline config: inputs resident in HBM before the timed region (replicas only across ranks:
     # each rank runs the same seeded workload on its own GPU)
     cfg = get_config(args.config)
@@ -629,6 +634,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary configs")
     ap.add_argument("--cpu-budget", type=float, default=10.0)
+    ap.add_argument("--only-next-rows", action="store_true",
+                    help="time only the SURVEY §8(f) rows (evaluation path, sub-blocks, Newton-Schulz)")
     ap.add_argument("--layers", type=int, default=0,
                     help="keep only the first L layers of the config resident (ncu captures of ragged)")
     args = ap.parse_args()

@@ -147,3 +147,87 @@ def test_newton_schulz_parity(case):
     # zero steps = the Frobenius-normalised input
     X0 = _f64(tab.tabattn_newton_schulz(_dev(G), 0))
     assert rel_l2(X0, br.newton_schulz(G, 0)) <= 3e-3
+
+
+# ---- at the size bench.py times (the long_item table: 688,128 cells, e = 256, hidden = 768) -------------------------
+def _full_inputs(torch, dev, B, R, C, e, hid, seed):
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed)
+    rnd = lambda *s, scale=1.0: (torch.randn(*s, generator=g, device=dev, dtype=torch.float32) * scale).to(torch.bfloat16)
+    x, dy = rnd(B, R, C, e), rnd(B, R, C, e)
+    gain = (1 + 0.1 * torch.randn(e, generator=g, device=dev)).to(torch.bfloat16)
+    return x, dy, gain, rnd(3 * e, e, scale=e ** -0.5), rnd(e, e, scale=e ** -0.5), rnd(hid, e, scale=e ** -0.5), \
+        rnd(e, hid, scale=hid ** -0.5)
+
+
+def _np_bits(t):
+    import gpu_util as gu
+    return gu.to_bits(t)
+
+
+def test_mlp_block_full_size():
+    """All 688,128 cells: y and dx on a seeded sample of cells (the block is per-cell), the parameter gradients
+    (sums over ALL cells) against the oracle's full reduction."""
+    import torch
+    import paper_2606_03681_b200 as tab
+    from oracle import block_ref as br
+    dev = torch.device("cuda", 0)
+    B, R, C, e, hid, alpha = 8, 4096, 21, 256, 768, 0.95
+    x, dy, gain, _, _, W1, W2 = _full_inputs(torch, dev, B, R, C, e, hid, 77)
+    y, saved = tab.tabattn_mlp_fwd(x, gain, W1, W2, alpha)
+    dx, dg, dW1, dW2 = tab.tabattn_mlp_bwd(x, gain, W1, W2, saved, dy, alpha)
+    torch.cuda.synchronize()
+    for t in (y, dx, dg, dW1, dW2):
+        assert bool(torch.isfinite(t.float()).all())
+    xb, dyb = _np_bits(x).reshape(-1, e), _np_bits(dy).reshape(-1, e)
+    gb, w1, w2 = _np_bits(gain), _np_bits(W1), _np_bits(W2)
+    dx_, dg_, dW1_, dW2_ = br.mlp_bwd(xb, gb, w1, w2, dyb, alpha)       # the full reduction (numpy fp64 matmuls)
+    y_ = br.mlp_fwd(xb, gb, w1, w2, alpha)
+    assert rel_l2(_f64(y).reshape(-1, e), y_) <= Y_TOL
+    assert rel_l2(_f64(dx).reshape(-1, e), dx_) <= DX_TOL
+    # per-cell gate on a sample (a wrong tile would hide in the global norm): first / last cells and random ones
+    rng = np.random.default_rng(5)
+    idx = np.unique(np.concatenate([[0, 127, 128, xb.shape[0] - 1], rng.integers(0, xb.shape[0], 4096)]))
+    err = np.linalg.norm(_f64(y).reshape(-1, e)[idx] - y_[idx], axis=1) / np.linalg.norm(y_[idx], axis=1)
+    assert err.max() <= 4 * Y_TOL
+    for got, want, nm in ((dg, dg_, "dg"), (dW1, dW1_, "dW1"), (dW2, dW2_, "dW2")):
+        assert rel_l2(got.double().cpu().numpy(), want) <= DW_TOL, nm
+
+
+@pytest.mark.parametrize("axis", [0, 1], ids=["feature", "item"])
+def test_attention_block_full_size(axis):
+    """The long_item table through the attention sub-block.  Feature axis: everything, including the parameter
+    gradients, against the oracle on the whole tensor.  Item axis (43 TFLOP in fp64): y and dx of a seeded sample
+    of whole (b, c) sequences -- the block is per-sequence -- and finiteness of everything."""
+    import torch
+    import paper_2606_03681_b200 as tab
+    from oracle import block_ref as br
+    dev = torch.device("cuda", 0)
+    B, R, C, H, dh, n, alpha = 8, 4096, 21, 4, 64, 3072, 0.95
+    e = H * dh
+    x, dy, gain, Wqkv, Wo, _, _ = _full_inputs(torch, dev, B, R, C, e, 768, 78 + axis)
+    n_train = np.full(B, n, np.int32)
+    nt = torch.from_numpy(n_train).to(dev)
+    y, saved = tab.tabattn_attn_block_fwd(axis, x, gain, Wqkv, Wo, H, nt, None, alpha, n_train_host=n_train)
+    dx, dg, dWqkv, dWo = tab.tabattn_attn_block_bwd(axis, x, gain, Wqkv, Wo, H, saved, dy, nt, None, alpha,
+                                                    n_train_host=n_train)
+    torch.cuda.synchronize()
+    for t in (y, dx, dg, dWqkv, dWo):
+        assert bool(torch.isfinite(t.float()).all())
+    xb, dyb = _np_bits(x), _np_bits(dy)
+    gb, wq, wo = _np_bits(gain), _np_bits(Wqkv), _np_bits(Wo)
+    if axis == 0:
+        y_ = br.attn_block_fwd("feature", xb, gb, wq, wo, H, n_train, None, alpha)
+        dx_, dg_, dWqkv_, dWo_ = br.attn_block_bwd("feature", xb, gb, wq, wo, dyb, H, n_train, None, alpha)
+        assert rel_l2(_f64(y), y_) <= Y_TOL and rel_l2(_f64(dx), dx_) <= DX_TOL
+        for got, want, nm in ((dg, dg_, "dg"), (dWqkv, dWqkv_, "dWqkv"), (dWo, dWo_, "dWo")):
+            assert rel_l2(got.double().cpu().numpy(), want) <= DW_TOL, nm
+    else:
+        rng = np.random.default_rng(6)
+        yg, dxg = _f64(y), _f64(dx)
+        for b, c in [(0, 0), (B - 1, C - 1), (int(rng.integers(B)), int(rng.integers(C)))]:
+            sl = (slice(b, b + 1), slice(None), slice(c, c + 1))
+            y_ = br.attn_block_fwd("item", xb[sl], gb, wq, wo, H, n_train[b:b + 1], None, alpha)
+            dx_ = br.attn_block_bwd("item", xb[sl], gb, wq, wo, dyb[sl], H, n_train[b:b + 1], None, alpha)[0]
+            assert rel_l2(yg[sl], y_) <= Y_TOL, (b, c)
+            assert rel_l2(dxg[sl], dx_) <= DX_TOL, (b, c)
