@@ -14,24 +14,38 @@ namespace tabattn {
 
 namespace {
 
-constexpr int kNormWarps = 8;        // rows per CTA pass of the RMSNorm kernels
-constexpr int kMaxChunks = 4;        // 16-byte chunks per lane: e <= 1024
+constexpr int kNormWarps = 8;        // warps per CTA of the RMSNorm kernels
+constexpr int kNormRows = 4;         // rows a warp has in flight (independent 16-byte loads per lane)
 
-// h = rmsnorm(alpha x) o g (bf16), rstd = 1 / sqrt(mean((alpha x)^2) + eps) (fp32); one warp per row
+// The RMSNorm kernels are pure streams (2-5 passes over [cells][e]); a warp owns whole rows, a lane CPL 16-byte
+// chunks of each (CPL = ceil(e / 256): 1 for the model widths 192 and 256), and works on kNormRows rows at once so
+// that enough loads are in flight (profiles/r02_blocks.md: one row per warp reached 30 % / 20 % of HBM).
+
+// h = rmsnorm(alpha x) o g (bf16), rstd = 1 / sqrt(mean((alpha x)^2) + eps) (fp32)
+template <int CPL>
 __global__ void __launch_bounds__(kNormWarps * 32)
 rmsnorm_fwd_kernel(const uint4* __restrict__ x, const uint4* __restrict__ g, uint4* __restrict__ h,
                    float* __restrict__ rstd, long long M, int e, float alpha, float eps) {
   const int lane = threadIdx.x & 31, chunks = e >> 3;
-  float gv[kMaxChunks][8];
+  float gv[CPL][8];
 #pragma unroll
-  for (int q = 0; q < kMaxChunks; ++q)
+  for (int q = 0; q < CPL; ++q)
     if (lane + 32 * q < chunks) unpack8(__ldg(g + lane + 32 * q), gv[q]);
-  for (long long m = (long long)blockIdx.x * kNormWarps + (threadIdx.x >> 5); m < M; m += (long long)gridDim.x * kNormWarps) {
-    float v[kMaxChunks][8], ss = 0.f;
+  const long long stride = (long long)gridDim.x * kNormWarps * kNormRows;
+  for (long long m0 = ((long long)blockIdx.x * kNormWarps + (threadIdx.x >> 5)) * kNormRows; m0 < M; m0 += stride) {
+    uint4 raw[kNormRows][CPL];
 #pragma unroll
-    for (int q = 0; q < kMaxChunks; ++q)
-      if (lane + 32 * q < chunks) {
-        unpack8(ldg_nc_v4(x + m * chunks + lane + 32 * q), v[q]);
+    for (int r = 0; r < kNormRows; ++r)
+#pragma unroll
+      for (int q = 0; q < CPL; ++q)
+        raw[r][q] = (m0 + r < M && lane + 32 * q < chunks) ? ldg_nc_v4(x + (m0 + r) * chunks + lane + 32 * q)
+                                                            : make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int r = 0; r < kNormRows; ++r) {
+      float v[CPL][8], ss = 0.f;
+#pragma unroll
+      for (int q = 0; q < CPL; ++q) {
+        unpack8(raw[r][q], v[q]);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           v[q][k] *= alpha;
@@ -39,68 +53,92 @@ rmsnorm_fwd_kernel(const uint4* __restrict__ x, const uint4* __restrict__ g, uin
         }
       }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-    const float r = rsqrtf(ss / (float)e + eps);
-    if (lane == 0) rstd[m] = r;
+      for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+      const float rs = rsqrtf(ss / (float)e + eps);
+      if (m0 + r < M) {
+        if (lane == 0) rstd[m0 + r] = rs;
 #pragma unroll
-    for (int q = 0; q < kMaxChunks; ++q)
-      if (lane + 32 * q < chunks) {
-        float o[8];
+        for (int q = 0; q < CPL; ++q)
+          if (lane + 32 * q < chunks) {
+            float o[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) o[k] = v[q][k] * r * gv[q][k];
-        stg_v4(h + m * chunks + lane + 32 * q, pack8(o));
+            for (int k = 0; k < 8; ++k) o[k] = v[q][k] * rs * gv[q][k];
+            stg_v4(h + (m0 + r) * chunks + lane + 32 * q, pack8(o));
+          }
       }
+    }
   }
 }
 
 // Backward of  xs = alpha x,  h = xs rstd o g,  out = xs + f(h):  given dh and dy (the gradient of `out`),
 //   t = dh o g,  xh = xs rstd,  dxs = dy + rstd (t - xh mean(t o xh)),  dx = alpha dxs,  dg += dh o xh.
 // dg: per-warp register sums over the warp's rows, then one partial row per CTA (reduced by colsum_kernel).
+template <int CPL>
 __global__ void __launch_bounds__(kNormWarps * 32)
 rmsnorm_bwd_kernel(const uint4* __restrict__ x, const uint4* __restrict__ g, const float* __restrict__ rstd,
                    const uint4* __restrict__ dh, const uint4* __restrict__ dy, uint4* __restrict__ dx,
                    float* __restrict__ dg_partial, long long M, int e, float alpha) {
-  __shared__ float sdg[kNormWarps][1024];
+  __shared__ float sdg[kNormWarps][CPL * 256];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, chunks = e >> 3;
-  float gv[kMaxChunks][8], acc[kMaxChunks][8];
+  constexpr int RB = 2;   // rows in flight (three streams each)
+  float gv[CPL][8], acc[CPL][8];
 #pragma unroll
-  for (int q = 0; q < kMaxChunks; ++q) {
+  for (int q = 0; q < CPL; ++q) {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) acc[q][k] = 0.f;
+    for (int k = 0; k < 8; ++k) acc[q][k] = gv[q][k] = 0.f;   // (lanes beyond the row contribute exact zeros)
     if (lane + 32 * q < chunks) unpack8(__ldg(g + lane + 32 * q), gv[q]);
   }
-  for (long long m = (long long)blockIdx.x * kNormWarps + warp; m < M; m += (long long)gridDim.x * kNormWarps) {
-    const float r = __ldg(rstd + m);
-    float xh[kMaxChunks][8], t[kMaxChunks][8], c = 0.f;
+  const long long stride = (long long)gridDim.x * kNormWarps * RB;
+  for (long long m0 = ((long long)blockIdx.x * kNormWarps + warp) * RB; m0 < M; m0 += stride) {
+    uint4 rx[RB][CPL], rh[RB][CPL], ry[RB][CPL];
+    float rr[RB];
 #pragma unroll
-    for (int q = 0; q < kMaxChunks; ++q)
-      if (lane + 32 * q < chunks) {
+    for (int r = 0; r < RB; ++r) {
+      const bool ok = m0 + r < M;
+      rr[r] = ok ? __ldg(rstd + m0 + r) : 0.f;
+#pragma unroll
+      for (int q = 0; q < CPL; ++q) {
+        const bool in = ok && lane + 32 * q < chunks;
+        const long long i = (m0 + r) * chunks + lane + 32 * q;
+        rx[r][q] = in ? ldg_nc_v4(x + i) : make_uint4(0, 0, 0, 0);
+        rh[r][q] = in ? ldg_nc_v4(dh + i) : make_uint4(0, 0, 0, 0);
+        ry[r][q] = in ? ldg_nc_v4(dy + i) : make_uint4(0, 0, 0, 0);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      float xh[CPL][8], t[CPL][8], c = 0.f;
+#pragma unroll
+      for (int q = 0; q < CPL; ++q) {
         float d[8];
-        unpack8(ldg_nc_v4(x + m * chunks + lane + 32 * q), xh[q]);
-        unpack8(ldg_nc_v4(dh + m * chunks + lane + 32 * q), d);
+        unpack8(rx[r][q], xh[q]);
+        unpack8(rh[r][q], d);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          xh[q][k] *= alpha * r;
+          xh[q][k] *= alpha * rr[r];
           acc[q][k] = fmaf(d[k], xh[q][k], acc[q][k]);
           t[q][k] = d[k] * gv[q][k];
           c = fmaf(t[q][k], xh[q][k], c);
         }
       }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    c /= (float)e;
+      for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+      c /= (float)e;
+      if (m0 + r < M) {
 #pragma unroll
-    for (int q = 0; q < kMaxChunks; ++q)
-      if (lane + 32 * q < chunks) {
-        float d[8], o[8];
-        unpack8(ldg_nc_v4(dy + m * chunks + lane + 32 * q), d);
+        for (int q = 0; q < CPL; ++q)
+          if (lane + 32 * q < chunks) {
+            float d[8], o[8];
+            unpack8(ry[r][q], d);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) o[k] = alpha * (d[k] + r * (t[q][k] - xh[q][k] * c));
-        stg_v4(dx + m * chunks + lane + 32 * q, pack8(o));
+            for (int k = 0; k < 8; ++k) o[k] = alpha * (d[k] + rr[r] * (t[q][k] - xh[q][k] * c));
+            stg_v4(dx + (m0 + r) * chunks + lane + 32 * q, pack8(o));
+          }
       }
+    }
   }
 #pragma unroll
-  for (int q = 0; q < kMaxChunks; ++q)
+  for (int q = 0; q < CPL; ++q)
     if (lane + 32 * q < chunks) {
 #pragma unroll
       for (int k = 0; k < 8; ++k) sdg[warp][8 * (lane + 32 * q) + k] = acc[q][k];
@@ -156,6 +194,33 @@ int norm_grid(long long M, int num_sms) {
   const long long want = (M + kNormWarps - 1) / kNormWarps;
   const long long cap = (long long)num_sms * 8;
   return (int)(want < cap ? want : cap);
+}
+
+void launch_rmsnorm_fwd(const void* x, const void* g, void* h, float* rstd, long long M, int e, float alpha, float eps,
+                        int num_sms, cudaStream_t stream) {
+  const int grid = norm_grid(M, num_sms), cpl = (e / 8 + 31) / 32;
+  auto args = [&](auto kern) {
+    kern<<<grid, kNormWarps * 32, 0, stream>>>((const uint4*)x, (const uint4*)g, (uint4*)h, rstd, M, e, alpha, eps);
+  };
+  if (cpl <= 1) args(rmsnorm_fwd_kernel<1>);
+  else if (cpl == 2) args(rmsnorm_fwd_kernel<2>);
+  else args(rmsnorm_fwd_kernel<4>);
+  count_launch();
+}
+
+// returns the number of partial rows written to dg_partial
+int launch_rmsnorm_bwd(const void* x, const void* g, const float* rstd, const void* dh, const void* dy, void* dx,
+                       float* dg_partial, long long M, int e, float alpha, int num_sms, cudaStream_t stream) {
+  const int grid = norm_grid(M, num_sms), cpl = (e / 8 + 31) / 32;
+  auto args = [&](auto kern) {
+    kern<<<grid, kNormWarps * 32, 0, stream>>>((const uint4*)x, (const uint4*)g, rstd, (const uint4*)dh,
+                                                (const uint4*)dy, (uint4*)dx, dg_partial, M, e, alpha);
+  };
+  if (cpl <= 1) args(rmsnorm_bwd_kernel<1>);
+  else if (cpl == 2) args(rmsnorm_bwd_kernel<2>);
+  else args(rmsnorm_bwd_kernel<4>);
+  count_launch();
+  return grid;
 }
 
 gemm::Problem linear_problem(long long M, int N, int K) {
@@ -219,9 +284,7 @@ cudaError_t launch_mlp_fwd(long long cells, int e, int hidden, float alpha, floa
                            cudaStream_t stream) {
   const DeviceInfo* di = current_device();
   if (!di) return cudaErrorInvalidDevice;
-  rmsnorm_fwd_kernel<<<norm_grid(cells, di->num_sms), kNormWarps * 32, 0, stream>>>(
-      (const uint4*)x, (const uint4*)g, (uint4*)h, rstd, cells, e, alpha, eps);
-  count_launch();
+  launch_rmsnorm_fwd(x, g, h, rstd, cells, e, alpha, eps, di->num_sms, stream);
   // u = h W1^T (saved), a = gelu(u) (saved): one GEMM, two outputs
   gemm::Problem p1 = nt(h, cells, e, W1, hidden, u);
   p1.C[1] = a;
@@ -261,11 +324,9 @@ cudaError_t launch_mlp_bwd(long long cells, int e, int hidden, float alpha, cons
   // dh = du W1
   gemm::Problem q = nn(du, cells, hidden, W1, e, dh);
   if ((er = gemm::launch(q, stream)) != cudaSuccess) return er;
-  const int grid = norm_grid(cells, di->num_sms);
-  rmsnorm_bwd_kernel<<<grid, kNormWarps * 32, 0, stream>>>((const uint4*)x, (const uint4*)g, rstd, (const uint4*)dh,
-                                                            (const uint4*)dy, (uint4*)dx, dg_partial, cells, e, alpha);
+  const int grid = launch_rmsnorm_bwd(x, g, rstd, dh, dy, dx, dg_partial, cells, e, alpha, di->num_sms, stream);
   colsum_kernel<<<(e + 127) / 128, 128, 0, stream>>>(dg_partial, grid, e, dg);
-  count_launch(2);
+  count_launch();
   return cudaGetLastError();
 }
 
@@ -277,9 +338,7 @@ cudaError_t launch_attn_block_fwd(const Shape& s, int axis, float alpha, float e
   if (!di) return cudaErrorInvalidDevice;
   const long long cells = (long long)s.B * s.R * s.C;
   const int e = s.H * s.dh;
-  rmsnorm_fwd_kernel<<<norm_grid(cells, di->num_sms), kNormWarps * 32, 0, stream>>>(
-      (const uint4*)x, (const uint4*)g, (uint4*)h, rstd, cells, e, alpha, eps);
-  count_launch();
+  launch_rmsnorm_fwd(x, g, h, rstd, cells, e, alpha, eps, di->num_sms, stream);
   // [q | k | v] = h Wqkv^T, written as three [cells][e] tensors (the attention kernels' layout)
   gemm::Problem p = nt(h, cells, e, Wqkv, 3 * e, q);
   p.C[1] = k; p.C[2] = v;
@@ -349,11 +408,9 @@ cudaError_t launch_attn_block_bwd(const Shape& s, int axis, float alpha, const v
   r.B = {Wqkv, 1, e, 0};
   r.C[0] = dh; r.ldc = e;
   if ((er = gemm::launch(r, stream)) != cudaSuccess) return er;
-  const int grid = norm_grid(cells, di->num_sms);
-  rmsnorm_bwd_kernel<<<grid, kNormWarps * 32, 0, stream>>>((const uint4*)x, (const uint4*)g, rstd, (const uint4*)dh,
-                                                            (const uint4*)dy, (uint4*)dx, dg_partial, cells, e, alpha);
+  const int grid = launch_rmsnorm_bwd(x, g, rstd, dh, dy, dx, dg_partial, cells, e, alpha, di->num_sms, stream);
   colsum_kernel<<<(e + 127) / 128, 128, 0, stream>>>(dg_partial, grid, e, dg);
-  count_launch(2);
+  count_launch();
   return cudaGetLastError();
 }
 

@@ -78,11 +78,15 @@ struct Cfg {
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE = A_BYTES + B_BYTES;
   static constexpr int STAGING = (BN / 64) * (BM * 128);
-  static constexpr int SMEM = ST * STAGE + STAGING + 1024;
+  // the epilogue's staging tile: its own buffer when an auxiliary tile is prefetched into it, else it aliases the
+  // (by then idle) A stages, which lets a third CTA fit an SM
+  static constexpr int SMEM_AUX = ST * STAGE + STAGING + 1024;
+  static constexpr int SMEM_MAIN = ST * STAGE + 1024;
+  static_assert(STAGING <= ST * A_BYTES, "staging aliases the A stages");
 };
 
 template <int BN, int A_MN, int B_MN>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, 3)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA2,
                const __grid_constant__ CUtensorMap mapA3, const __grid_constant__ CUtensorMap mapB,
                const __grid_constant__ CUtensorMap mapAux, const __grid_constant__ CUtensorMap mapC0,
@@ -92,7 +96,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   constexpr int ST = C::ST;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sA = sbase, sB = sA + ST * A_BYTES, sOut = sB + ST * C::B_BYTES;
+  const uint32_t sA = sbase, sB = sA + ST * A_BYTES;
+  const uint32_t sOut = p.aux_mode != AUX_NONE ? sB + ST * C::B_BYTES : sA;
   __shared__ uint64_t bar_full[ST], bar_empty[ST], bar_acc, bar_aux;
   __shared__ uint32_t tmem_slot;
 
@@ -334,10 +339,11 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   if (!ok) return cudaErrorInvalidValue;
   auto kern = gemm_tc_kernel<BN, A_MN, B_MN>;
   static SmemAttr attr;
-  cudaError_t e = attr.ensure(kern, Cfg<BN>::SMEM, di->ordinal);
+  cudaError_t e = attr.ensure(kern, Cfg<BN>::SMEM_AUX, di->ordinal);
   if (e != cudaSuccess) return e;
+  const int smem = p.aux_mode != AUX_NONE ? Cfg<BN>::SMEM_AUX : Cfg<BN>::SMEM_MAIN;
   dim3 grid((p.N + BN - 1) / BN, (p.M + BM - 1) / BM, p.partial ? kp.slabs : p.batch);
-  kern<<<grid, kThreads, Cfg<BN>::SMEM, stream>>>(ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
+  kern<<<grid, kThreads, smem, stream>>>(ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
   count_launch();
   return cudaGetLastError();
 }
