@@ -11,7 +11,7 @@
 // there.  A softmax thread owns one slot (one TMEM lane) and reads only the W = max(Cp, 32) score columns
 // around its own block.  The tensor pipe is < 5 % busy on this axis, so the wasted off-diagonal flops are
 // free; what the packing buys is ~100 instead of ~460-930 warp instructions per (row, head) and bulk
-// TMA traffic, i.e. a kernel that is HBM-bound instead of issue-bound (profiles/r02_feature_tc.md).
+// TMA traffic, i.e. a kernel that is HBM-bound instead of issue-bound (profiles/r02_attention.md).
 //
 // Unmasked tables are one "virtual table" of B*R rows (every row has the same columns), fetched and
 // stored by 4-D TMA boxes (dh, 1 head, Cp columns, RPT rows): columns >= C are zero-filled on load and

@@ -85,7 +85,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
   __shared__ uint32_t tmem_slot;
   // -LSE log2(e) of every slot of a staged tile (+inf -> P = 0 for dead slots), written by the producer warps with
   // the tile: the softmax threads used to fetch it themselves one tile ahead, which cost them a register they
-  // did not have (the value was spilled right behind the load: 19 % of their time, profiles/r02_feature.md)
+  // did not have (the value was spilled right behind the load: 19 % of their time, profiles/r02_attention.md)
   __shared__ float sNL2[ST][kSlots];
   const Shape& s = p.s;
 
@@ -430,7 +430,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         // The single P/dS buffer is the serial section of the kernel (a tile holds it from its first store to
         // the completion of its accumulation MMAs), so everything that can be computed before the tile's turn
         // is: for W <= 64 the dS chunks wait in registers and the turn only covers the stores
-        // (profiles/r02_feature.md: the turn wait was 20 % of the softmax warps' samples at base).
+        // (profiles/r02_attention.md: the turn wait was 20 % of the softmax warps' samples at base).
         constexpr bool PRE = NCH <= 2;
         uint32_t dsr[PRE ? 16 * NCH : 16];
         if constexpr (PRE) {

@@ -31,7 +31,7 @@
 // Every role walks the same item list with its own counters.  The issuing warps run convergently with a
 // provably warp-uniform warp index, so ptxas keeps descriptors in uniform registers (~3 SASS instructions
 // per tcgen05.mma; the earlier builds needed ~10-20 and were bound by the issue chain,
-// profiles/r01_tc_launches.md, r01_s7_full.md, r01_s14_item.md).
+// profiles/r01_s14_item.md).
 #include <cuda.h>
 
 #include <algorithm>

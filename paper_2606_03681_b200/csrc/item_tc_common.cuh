@@ -47,7 +47,7 @@ struct Meta {
 // Incremental decode of the work items w = blockIdx.x + k * gridDim.x, w = ((b*C + c)*H + h)*bps + blk: the
 // six integer divisions of a direct decode are paid once; next() is ~15 adds/compares with carries.  (At base the
 // items are 6-16 inner tiles long and the direct decode plus the loads that depend on it were ~12 % of the score
-// warps' samples, profiles/r01_s27_final.md.)  seqmod = (sequence index) % bps serves the dK/dV block rotation.
+// warps' samples, profiles/r01_s46_final.md.)  seqmod = (sequence index) % bps serves the dK/dV block rotation.
 struct ItemCoord {
   int w, blk, h, c, b, seqmod;
   int s_blk, s_h, s_c, s_b, s_seqmod;   // per-step increments (step = gridDim.x items)

@@ -123,7 +123,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       // V tail fix; warp 10 / 11: O_t += P_t V_j for query tile t = 0 / 1.  Each warp runs its loop
       // convergently (elect.sync inside every issue) on precomputed descriptors.  One issuing warp costs
       // ~65 clk per tcgen05.mma (a dependent chain of ~10 SASS instructions), which bound the first two
-      // builds of this kernel (profiles/r01_s7_full.md, r01_s14_item.md); three warps in parallel do not.
+      // builds of this kernel (profiles/r01_s14_item.md); three warps in parallel do not.
       constexpr uint32_t TILE16 = TILE >> 4;
       uint32_t st = 0, ph = 0, par = 0, j = 0, tiles = 0, k = 0;
       int n = 0;

@@ -233,7 +233,7 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
 // comes back unchanged, but through an instruction that consumes the arrive's state token, so arithmetic that
 // uses the result cannot be scheduled above the arrive.  Without this ptxas sinks the arrive that releases a
 // TMEM buffer under most of the arithmetic on the loaded registers (it has no data dependency on it), which
-// delays the next MMAs into that buffer by most of a chunk's compute time (profiles/r01_s27_final.md).
+// delays the next MMAs into that buffer by most of a chunk's compute time (profiles/r01_s46_final.md).
 __device__ __forceinline__ float mbar_arrive_then(uint32_t bar, uint32_t do_arrive, float carry) {
   asm volatile(
       "{\n\t.reg .b64 st;\n\t.reg .b32 lo, hi;\n\t.reg .pred q, p;\n\t"
