@@ -168,7 +168,7 @@ __device__ __forceinline__ void zero_invalid_cells(const FeatParams& p, unsigned
       }
       if (lse)
         for (uint32_t i = lane; i < (uint32_t)ninv * s.H; i += 32) {
-          const uint32_t h = __umulhi(i, m_ni), kk = i - h * ninv;
+          const uint32_t h = ninv == 1 ? i : __umulhi(i, m_ni), kk = i - h * ninv;   // (the magic number is 2^32 at ninv = 1)
           lse[(row * s.H + h) * s.C + __ldg(inv + kk)] = 0.f;
         }
     }

@@ -122,11 +122,11 @@ __device__ __forceinline__ void softmax_window(uint32_t tSwin, uint32_t tProw, i
     tmem_wait_ld();
     const float* sf = reinterpret_cast<const float*>(sr);
 #pragma unroll
-    for (int k = 0; k < 32; k += 4) {
-      mx0 = fmaxf(mx0, sf[k]);
-      mx1 = fmaxf(mx1, sf[k + 1]);
-      mx2 = fmaxf(mx2, sf[k + 2]);
-      mx3 = fmaxf(mx3, sf[k + 3]);
+    for (int k = 0; k < 32; k += 8) {
+      mx0 = fmax3(mx0, sf[k], sf[k + 1]);
+      mx1 = fmax3(mx1, sf[k + 2], sf[k + 3]);
+      mx2 = fmax3(mx2, sf[k + 4], sf[k + 5]);
+      mx3 = fmax3(mx3, sf[k + 6], sf[k + 7]);
     }
   }
   // every slot sees at least one live key of its own block (bias 0), so the maximum is a real score

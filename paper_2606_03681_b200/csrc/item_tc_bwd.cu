@@ -61,12 +61,23 @@ struct BwdCfg {
   static constexpr int TILE_B = kChunk * ROWB;     // streamed chunk
   // chunk ring depth: as deep as shared memory allows at dh = 64 (8 stages, 196 KB); 16 at dh <= 32 (B200 sweep:
   // base bwd 1.451 / 1.436 / 1.414 / 1.404 / 1.418 ms at 6 / 8 / 12 / 16 / 20 stages, 1.586 at 4)
-  static constexpr int ST = DH >= 64 ? 8 : 16;
-  static constexpr int LD_BYTES = 2 * kChunk * 4;  // per stage: lse2[64], D[64] (MODE_DKV)
+  // FOLD: `dP - D` is computed by the dP MMA itself (one extra k-step, see `D records` below) instead of a
+  // subtraction per score element in the issue-bound score loops of dh <= 32 (profiles/r02_attention.md: issue
+  // 76 % / 70 %, XU 56 % / 43 %).  At dh = 64 the tensor pipe is as busy as the MUFU and the loop is not issue-bound.
+  static constexpr bool FOLD = DH <= 32;
+  static constexpr int ST = DH >= 64 ? 8 : 12;
+  static constexpr int LD_BYTES = 2 * kChunk * 4;  // per stage: lse2[64], D[64] (MODE_DKV; D unused with FOLD)
   static constexpr int STAGE = 2 * TILE_B;         // bytes of one ring stage (B1, B2)
   static constexpr int STAT_BYTES = 2 * 2 * kTileRows * 4;   // MODE_DQ: [2 item buffers][nlse2[128], D[128]]
+  // D records (FOLD): one 32-byte row per query, (-D_hi, -D_lo, 0 x 14) bf16 in the 32-byte-swizzle K-major layout,
+  // so that a [rows][16] tile of them is an MMA operand: against a tile of (1, 1, 0 x 14) rows the product is -D.
+  static constexpr int REC = 32;
+  static constexpr int ONES_BYTES = kTileRows * REC;                 // the (1, 1, 0...) operand
+  static constexpr int DA_BYTES = 2 * kTileRows * REC;               // MODE_DQ: [2 item buffers][128 query rows]
+  static constexpr int DB_BYTES = kChunk * REC;                      // MODE_DKV: per stage, the chunk's 64 queries
+  static constexpr int FOLD_BYTES = FOLD ? ONES_BYTES + DA_BYTES + ST * DB_BYTES : 0;
   // (+ one O tile in MODE_DQ; sized for the larger of the two modes)
-  static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + TILE_A + STAT_BYTES + 1024;
+  static constexpr int SMEM = 4 * TILE_A + ST * (STAGE + LD_BYTES) + TILE_A + STAT_BYTES + FOLD_BYTES + 1024;
   // TMEM columns: set g at g*SET: S [0,64) dP [64,128) dS [128,160) P [160,192); accumulators after
   static constexpr int SET = 192, S_OFF = 0, DP_OFF = 64, DS_OFF = 128, P_OFF = 160;
   static constexpr int ACC0 = 384, ACC1 = 384 + DH, COLS = 512;
@@ -111,7 +122,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1)
 item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_constant__ CUtensorMap mapA2,
                    const __grid_constant__ CUtensorMap mapB1, const __grid_constant__ CUtensorMap mapB2,
                    const __grid_constant__ CUtensorMap mapO, Shape s, const float* __restrict__ LSE,
-                   float* lse2_ws, float* D_ws, __nv_bfloat16* __restrict__ out0,
+                   float* lse2_ws, float* D_ws, uint4* Drec_ws, __nv_bfloat16* __restrict__ out0,
                    __nv_bfloat16* __restrict__ out1, int n_items, int blocks_per_seq, int Rp) {
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE_A = Cfg::TILE_A, TILE_B = Cfg::TILE_B, ROWB = Cfg::ROWB;
@@ -122,6 +133,10 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   const uint32_t sLD = sB + ST * Cfg::STAGE;         // [ST][lse2[64], D[64]]
   const uint32_t sO = sLD + ST * Cfg::LD_BYTES;      // MODE_DQ: the item's O tile (single buffer)
   const uint32_t sStat = sO + TILE_A;                // MODE_DQ: [2][nlse2[128], D[128]]
+  constexpr bool FOLD = Cfg::FOLD;
+  const uint32_t sOnes = (sStat + Cfg::STAT_BYTES + 1023u) & ~1023u;   // FOLD: [128][32 B] rows (1, 1, 0...)
+  const uint32_t sDA = sOnes + Cfg::ONES_BYTES;      // FOLD, MODE_DQ: [2][128][32 B] D records of the item's queries
+  const uint32_t sDB = sDA + Cfg::DA_BYTES;          // FOLD, MODE_DKV: [ST][64][32 B] D records of the chunk's queries
   const float* sLD_ptr = reinterpret_cast<const float*>(smem_raw + (sLD - smem_u32(smem_raw)));
   float* sStat_ptr = reinterpret_cast<float*>(smem_raw + (sStat - smem_u32(smem_raw)));
   __shared__ uint64_t bar_a_full[2], bar_a_empty[2], bar_b_full[ST], bar_b_empty[ST];
@@ -155,6 +170,15 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     mbar_init(smem_u32(&bar_acc_full), kAccWarps(MODE));
     mbar_init(smem_u32(&bar_acc_free), (MODE == MODE_DQ && DH < 32) ? 8 : 16);   // warps that read the accumulators
     fence_barrier_init();
+  }
+  if (FOLD) {
+    // the (1, 1, 0 x 14) rows: k = 0..7 sit in the 16-byte half selected by the 32-byte swizzle (bit 2 of the row)
+    for (int r = threadIdx.x; r < kTileRows; r += blockDim.x) {
+      const uint32_t sw = (r >> 2) & 1;
+      sts_v4(sOnes + r * Cfg::REC + (sw << 4), 0x3F803F80u, 0u, 0u, 0u);
+      sts_v4(sOnes + r * Cfg::REC + ((sw ^ 1) << 4), 0u, 0u, 0u, 0u);
+    }
+    fence_proxy_async_smem();
   }
   tc_fence_before();
   __syncthreads();
@@ -192,12 +216,13 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         for (int j = 0; j < it.chunks; ++j, ++t) {
           const uint32_t st = t % ST, b_full = smem_u32(&bar_b_full[st]);
           mbar_wait<true>(smem_u32(&bar_b_empty[st]), ((t / ST) & 1) ^ 1);
-          mbar_arrive_expect_tx(b_full, Cfg::STAGE + (MODE == MODE_DKV ? Cfg::LD_BYTES : 0));
+          mbar_arrive_expect_tx(b_full, Cfg::STAGE + (MODE == MODE_DKV ? (FOLD ? kChunk * 4 + Cfg::DB_BYTES : Cfg::LD_BYTES) : 0));
           tma_load_5d(sB + st * Cfg::STAGE, &mapB1, b_full, 0, it.h, it.c, j * kChunk, it.b);
           tma_load_5d(sB + st * Cfg::STAGE + TILE_B, &mapB2, b_full, 0, it.h, it.c, j * kChunk, it.b);
           if (MODE == MODE_DKV) {
             bulk_load(sLD + st * Cfg::LD_BYTES, lse2_ws + seq + j * kChunk, kChunk * 4, b_full);
-            bulk_load(sLD + st * Cfg::LD_BYTES + kChunk * 4, D_ws + seq + j * kChunk, kChunk * 4, b_full);
+            if (FOLD) bulk_load(sDB + st * Cfg::DB_BYTES, Drec_ws + 2 * (seq + j * kChunk), Cfg::DB_BYTES, b_full);
+            else bulk_load(sLD + st * Cfg::LD_BYTES + kChunk * 4, D_ws + seq + j * kChunk, kChunk * 4, b_full);
           }
         }
         ++k;
@@ -211,6 +236,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     constexpr uint32_t idesc = make_idesc_bf16(128, kChunk, false, false);
     const uint64_t dA = make_smem_desc<ROWB>(sA, 16, 8 * ROWB);
     const uint64_t dB = make_smem_desc<ROWB>(sB, 16, 8 * ROWB);
+    const uint64_t dOnes = make_smem_desc<32>(sOnes, 16, 256), dRecA = make_smem_desc<32>(sDA, 16, 256),
+                   dRecB = make_smem_desc<32>(sDB, 16, 256);
     const uint32_t b_a_full = smem_u32(&bar_a_full[0]), b_a_empty = smem_u32(&bar_a_empty[0]),
                    b_b_full = smem_u32(&bar_b_full[0]), b_s_full = smem_u32(&bar_s_full[0]),
                    b_s_empty = smem_u32(&bar_s_empty[0]);
@@ -220,6 +247,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
       mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
+      // FOLD, dQ pass: the item's D records (written by the statistics warp) are the A operand of the extra k-step
+      if (FOLD && MODE == MODE_DQ) mbar_wait(smem_u32(&bar_d_full[ab]), (k >> 1) & 1);
       const uint64_t a1 = dA + ((2 * ab) * TILE_A >> 4), a2 = a1 + (TILE_A >> 4);
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
@@ -239,6 +268,11 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(set + Cfg::S_OFF, a1 + 2 * kk, b1 + 2 * kk, idesc, kk > 0);
 #pragma unroll
         for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(set + Cfg::DP_OFF, a2 + 2 * kk, b2 + 2 * kk, idesc, kk > 0);
+        if (FOLD) {
+          // dP -= D: (-D_hi, -D_lo) of the row (dQ pass: queries are rows) or of the column (dK/dV pass) times (1, 1)
+          if (MODE == MODE_DQ) mma_ss_e(set + Cfg::DP_OFF, dRecA + (ab * (kTileRows * Cfg::REC) >> 4), dOnes, idesc, 1u);
+          else mma_ss_e(set + Cfg::DP_OFF, dOnes, dRecB + (st * Cfg::DB_BYTES >> 4), idesc, 1u);
+        }
         tc_commit_e(b_s_full + 8 * g);
         if (j == it.chunks - 1) tc_commit_e(b_a_empty + 8 * ab);
         if (++st == ST) { st = 0; ph ^= 1; }
@@ -324,11 +358,26 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const int rr = lane + 32 * q, row = it.blk * kTileRows + rr;
+        const float Dv = st[kTileRows + rr];
+        if (FOLD) {
+          // -D as two bf16 (hi + lo carries 16 mantissa bits), in the half of the 32-byte row the swizzle selects
+          const uint32_t hi = pack_bf16(-Dv, 0.f) & 0xffffu;
+          const uint32_t lo = pack_bf16(-Dv - bf16lo(hi), 0.f) & 0xffffu;
+          const uint32_t sw = (rr >> 2) & 1;
+          sts_v4(sDA + ab * (kTileRows * Cfg::REC) + rr * Cfg::REC + (sw << 4), hi | (lo << 16), 0u, 0u, 0u);
+          sts_v4(sDA + ab * (kTileRows * Cfg::REC) + rr * Cfg::REC + ((sw ^ 1) << 4), 0u, 0u, 0u, 0u);
+          if (row < Rp) {
+            uint4* rec = Drec_ws + 2 * (seq * Rp + row);
+            rec[sw] = make_uint4(hi | (lo << 16), 0u, 0u, 0u);
+            rec[sw ^ 1] = make_uint4(0u, 0u, 0u, 0u);
+          }
+        }
         if (row < Rp) {
           lse2_ws[seq * Rp + row] = st[rr];
-          D_ws[seq * Rp + row] = st[kTileRows + rr];
+          if (!FOLD) D_ws[seq * Rp + row] = Dv;
         }
       }
+      if (FOLD) fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&bar_d_full[ab]));
       ++k;
@@ -458,7 +507,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
             const uint64_t x = fma2(f2pack(__uint_as_float(sr[2 * k]), __uint_as_float(sr[2 * k + 1])), cc, nl);
             float p0, p1, d0, d1;
             exp2_pair(pair_is_poly<Cfg::POLY_OF_8>(k), x, p0, p1);
-            const uint64_t dpd = sub2(f2pack(__uint_as_float(dr[2 * k]), __uint_as_float(dr[2 * k + 1])), dd);
+            uint64_t dpd = f2pack(__uint_as_float(dr[2 * k]), __uint_as_float(dr[2 * k + 1]));
+            if (!FOLD) dpd = sub2(dpd, dd);
             f2unpack(mul2(f2pack(p0, p1), dpd), d0, d1);
             pds[k] = pack_bf16(d0, d1);
           }
@@ -478,7 +528,9 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           const ulonglong2* d4 = l4 + kChunk / 4;
 #pragma unroll
           for (int k = 0; k < 32; k += 4) {
-            const ulonglong2 L = l4[k >> 2], Dv = d4[k >> 2];  // (nlse2, D) of query columns 32c + k .. k+3
+            const ulonglong2 L = l4[k >> 2];  // (nlse2, D) of query columns 32c + k .. k+3
+            ulonglong2 Dv = make_ulonglong2(0ull, 0ull);
+            if (!FOLD) Dv = d4[k >> 2];
             float p0, p1, p2, p3, d0, d1, d2, d3;
             const uint64_t xa = fma2(f2pack(__uint_as_float(sr[k]), __uint_as_float(sr[k + 1])), cc, L.x);
             const uint64_t xb = fma2(f2pack(__uint_as_float(sr[k + 2]), __uint_as_float(sr[k + 3])), cc, L.y);
@@ -486,8 +538,12 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
             exp2_pair(pair_is_poly<Cfg::POLY_OF_8>((k >> 1) + 1), xb, p2, p3);
             pp[k >> 1] = pack_bf16(p0, p1);
             pp[(k >> 1) + 1] = pack_bf16(p2, p3);
-            const uint64_t da = sub2(f2pack(__uint_as_float(dr[k]), __uint_as_float(dr[k + 1])), Dv.x);
-            const uint64_t db = sub2(f2pack(__uint_as_float(dr[k + 2]), __uint_as_float(dr[k + 3])), Dv.y);
+            uint64_t da = f2pack(__uint_as_float(dr[k]), __uint_as_float(dr[k + 1]));
+            uint64_t db = f2pack(__uint_as_float(dr[k + 2]), __uint_as_float(dr[k + 3]));
+            if (!FOLD) {
+              da = sub2(da, Dv.x);
+              db = sub2(db, Dv.y);
+            }
             f2unpack(mul2(f2pack(p0, p1), da), d0, d1);
             f2unpack(mul2(f2pack(p2, p3), db), d2, d3);
             pds[k >> 1] = pack_bf16(d0, d1);
@@ -541,13 +597,14 @@ cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void*
   if (e != cudaSuccess) return e;
   const int Rp = item_bwd_padded_rows(s);
   float* lse2_ws = ws;
-  float* D_ws = ws + (size_t)s.B * s.C * s.H * Rp;
+  float* D_ws = ws + (size_t)s.B * s.C * s.H * Rp;            // fp32 D per row (dh = 64) ...
+  uint4* Drec_ws = reinterpret_cast<uint4*>(D_ws);            // ... or one 32-byte D record per row (dh <= 32)
   const int bps = (s.R + kTileRows - 1) / kTileRows;
   const long long n_items = (long long)s.B * s.C * s.H * bps;
   const int grid = (int)std::min<long long>(n_items, di->num_sms);
-  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, o128, s, LSE, lse2_ws, D_ws,
+  kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, o128, s, LSE, lse2_ws, D_ws, Drec_ws,
                                                (__nv_bfloat16*)dQ, nullptr, (int)n_items, bps, Rp);
-  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, o128, s, LSE, lse2_ws, D_ws,
+  kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, o128, s, LSE, lse2_ws, D_ws, Drec_ws,
                                                 (__nv_bfloat16*)dV, (__nv_bfloat16*)dK, (int)n_items, bps, Rp);
   count_launch(2);
   return cudaGetLastError();
@@ -560,7 +617,9 @@ int item_bwd_padded_rows(const Shape& s) { return (s.R + kChunk - 1) / kChunk * 
 }  // namespace
 
 size_t item_bwd_workspace_bytes(const Shape& s) {
-  return (size_t)2 * s.B * s.C * s.H * item_bwd_padded_rows(s) * sizeof(float);
+  // per query row: -LSE log2(e) as f32, and D as f32 (dh = 64) or as a 32-byte operand record (dh <= 32, BwdCfg::FOLD)
+  const size_t per_row = sizeof(float) + (s.dh <= 32 ? 32 : sizeof(float));
+  return (size_t)s.B * s.C * s.H * item_bwd_padded_rows(s) * per_row;
 }
 
 cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
