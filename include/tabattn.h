@@ -98,7 +98,8 @@ TABATTN_API tabattn_status tabattn_item_fwd(const tabattn_shape* shape, const vo
 
 /* Item attention backward: a dQ pass (it also computes D = rowsum(dO o O) and -LSE*log2(e) per query
  * row and leaves them in the workspace) and a separate dK/dV pass that reads them; two kernel
- * launches, deterministic, no atomics.  ws: tabattn_workspace_bytes(shape, TABATTN_OP_ITEM_BWD). */
+ * launches, deterministic, no atomics.  ws: tabattn_workspace_bytes(shape, TABATTN_OP_ITEM_BWD)
+ * (8 bytes per (b, c, h, row) at dh = 64, 36 at dh <= 32, rows rounded up to 64). */
 TABATTN_API tabattn_status tabattn_item_bwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
                                 const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
                                 void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);

@@ -22,8 +22,9 @@ bool feature_shape_supported(const Shape& s);
 size_t feature_workspace_bytes(const Shape& s);   // masked calls: per-table geometry built by the a0 prep kernel
 
 // ---- item axis (item_tc_fwd.cu, item_tc_bwd.cu) ---------------------------------------------------------
-// The backward's workspace holds two f32 arrays [B*C*H][Rp] (Rp = R rounded up to 64): -LSE*log2(e) and
-// D = rowsum(dO o O), written by the dQ pass and read by the dK/dV pass.  The forward needs none.
+// The backward's workspace holds, per query row of [B*C*H][Rp] (Rp = R rounded up to 64), -LSE*log2(e) as f32 and
+// D = rowsum(dO o O) as f32 (dh = 64) or as a 32-byte MMA operand record (dh <= 32); written by the dQ pass and
+// read by the dK/dV pass.  The forward needs none.
 // query rows [q_row0, q_row1) of every sequence; LSE may be NULL (inference)
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                             int q_row0, int q_row1, cudaStream_t stream);
