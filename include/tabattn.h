@@ -55,6 +55,7 @@ typedef enum {
                                   n_train_host[b] outside [1,R], NULL shape, an output pointer equal
                                   to another argument's pointer (aliasing) */
   TABATTN_ERR_UNSUPPORTED = 2, /* dh not in {16,32,64}, C > TABATTN_MAX_FEATURE_C for feature_*,
+                                  B or C > 65535 for a masked item_* call,
                                   H*dh > TABATTN_MAX_D, B*R*C >= 2^31 cells, the calling thread's
                                   current device is not sm_100 */
   TABATTN_ERR_WORKSPACE = 3,   /* ws == NULL or ws_bytes < tabattn_workspace_bytes(shape, op) */
@@ -92,7 +93,8 @@ TABATTN_API tabattn_status tabattn_feature_bwd(const tabattn_shape* shape, const
                                    const void* O, const void* dO, const float* LSE, void* dQ, void* dK,
                                    void* dV, void* ws, size_t ws_bytes, tabattn_stream stream);
 
-/* Item attention forward.  LSE is [B,C,H,R] f32 (contiguous along the sequence). */
+/* Item attention forward.  LSE is [B,C,H,R] f32 (contiguous along the sequence).  ws (only touched when a
+ * column mask is given): tabattn_workspace_bytes(shape, TABATTN_OP_ITEM_FWD). */
 TABATTN_API tabattn_status tabattn_item_fwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
                                 void* O, float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream);
 

@@ -29,6 +29,8 @@ tabattn_status check_shape(const tabattn_shape* sh, bool item, Shape* out) {
   if (cells >= (1LL << 31) || (long long)sh->H * sh->dh > TABATTN_MAX_D) return TABATTN_ERR_UNSUPPORTED;
   if (item) {
     if (!sh->n_train) return TABATTN_ERR_INVALID_ARG;
+    // masked item calls pack (b, c) into 16 + 16 bits (the a0 column list)
+    if (sh->col_valid && (sh->B > 65535 || sh->C > 65535)) return TABATTN_ERR_UNSUPPORTED;
     if (sh->n_train_host)
       for (int b = 0; b < sh->B; ++b)
         if (sh->n_train_host[b] < 1 || sh->n_train_host[b] > sh->R) return TABATTN_ERR_INVALID_ARG;
@@ -106,6 +108,7 @@ size_t tabattn_workspace_bytes(const tabattn_shape* sh, int op) {
   if (check_shape(&tmp, op >= 2, &s) != TABATTN_OK) return 0;
   switch (op) {
     case TABATTN_OP_ITEM_BWD: return tabattn::item_bwd_workspace_bytes(s);
+    case TABATTN_OP_ITEM_FWD: return tabattn::item_fwd_workspace_bytes(s);
     case TABATTN_OP_FEATURE_FWD:
     case TABATTN_OP_FEATURE_BWD: return tabattn::feature_workspace_bytes(s);
     default: return 0;
@@ -152,15 +155,16 @@ tabattn_status tabattn_item_fwd(const tabattn_shape* sh, const void* Q, const vo
   Shape s;
   tabattn_status st = check_shape(sh, true, &s);
   if (st != TABATTN_OK) return st;
-  (void)ws; (void)ws_bytes;
   if (!all_ok(Q, K, V, (const void*)O, (const void*)LSE)) return TABATTN_ERR_INVALID_ARG;
   {
     const void* const outs[] = {O, LSE};
     const void* const ins[] = {Q, K, V};
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
+  // the workspace is only touched when a column mask is given (the a0 column list)
+  if (s.col_valid && (st = check_ws(tabattn::item_fwd_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, 0, s.R, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, 0, s.R, ws, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_feature_fwd_infer(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
@@ -185,15 +189,15 @@ tabattn_status tabattn_item_fwd_infer(const tabattn_shape* sh, const void* Q, co
   Shape s;
   tabattn_status st = check_shape(sh, true, &s);
   if (st != TABATTN_OK) return st;
-  (void)ws; (void)ws_bytes;
   if (!all_ok(Q, K, V, (const void*)O) || row0 < 0 || row1 <= row0 || row1 > s.R) return TABATTN_ERR_INVALID_ARG;
   {
     const void* const outs[] = {O};
     const void* const ins[] = {Q, K, V};
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
+  if (s.col_valid && (st = check_ws(tabattn::item_fwd_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
   if ((st = check_device()) != TABATTN_OK) return st;
-  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, nullptr, row0, row1, (cudaStream_t)stream));
+  return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, nullptr, row0, row1, ws, (cudaStream_t)stream));
 }
 
 tabattn_status tabattn_item_bwd(const tabattn_shape* sh, const void* Q, const void* K, const void* V,
@@ -232,7 +236,8 @@ size_t tabattn_attn_block_workspace_bytes(const tabattn_shape* sh, int32_t axis,
   if (check_shape(&tmp, axis == 1, &s) != TABATTN_OK) return 0;
   const tabattn::DeviceInfo* di = tabattn::current_device();
   const int sms = di ? di->num_sms : 148;
-  return backward ? tabattn::attn_block_bwd_ws_bytes(s, axis, sms) : tabattn::feature_workspace_bytes(s);
+  return backward ? tabattn::attn_block_bwd_ws_bytes(s, axis, sms)
+                  : (axis == 0 ? tabattn::feature_workspace_bytes(s) : tabattn::item_fwd_workspace_bytes(s));
 }
 
 tabattn_status tabattn_attn_block_fwd(const tabattn_shape* sh, int32_t axis, float alpha, float eps, const void* x,
@@ -251,7 +256,9 @@ tabattn_status tabattn_attn_block_fwd(const tabattn_shape* sh, int32_t axis, flo
     const void* const ins[] = {x, g, Wqkv, Wo};
     if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
   }
-  if (axis == 0 && s.col_valid && (st = check_ws(tabattn::feature_workspace_bytes(s), ws, ws_bytes)) != TABATTN_OK) return st;
+  if (s.col_valid && (st = check_ws(axis == 0 ? tabattn::feature_workspace_bytes(s) : tabattn::item_fwd_workspace_bytes(s), ws,
+                                    ws_bytes)) != TABATTN_OK)
+    return st;
   if ((st = check_device()) != TABATTN_OK) return st;
   return from_cuda(tabattn::launch_attn_block_fwd(s, axis, or_default(alpha, 1.f), or_default(eps, 1e-6f), x, g, Wqkv,
                                                   Wo, y, sv->h, sv->rstd, sv->q, sv->k, sv->v, sv->o, sv->lse, ws,

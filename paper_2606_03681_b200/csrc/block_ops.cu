@@ -346,7 +346,7 @@ cudaError_t launch_attn_block_fwd(const Shape& s, int axis, float alpha, float e
   cudaError_t er = gemm::launch(p, stream);
   if (er != cudaSuccess) return er;
   er = axis == 0 ? launch_feature_fwd(s, q, k, v, o, lse, ws, stream)
-                 : launch_item_fwd(s, q, k, v, o, lse, 0, s.R, stream);
+                 : launch_item_fwd(s, q, k, v, o, lse, 0, s.R, ws, stream);
   if (er != cudaSuccess) return er;
   // y = alpha x + o Wo^T
   gemm::Problem p2 = nt(o, cells, e, Wo, e, y);

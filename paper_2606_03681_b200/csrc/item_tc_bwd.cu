@@ -92,8 +92,8 @@ struct Item {
   bool valid;
 };
 
-template <int MODE>
-__device__ __forceinline__ Item decode_item(const Shape& s, const Meta& meta, int w, int bps) {
+template <int MODE, bool MASKED>
+__device__ __forceinline__ Item decode_item(const Shape& s, const Meta& meta, const ColList<MASKED>& cl, int w, int bps) {
   Item it;
   const int rest = w / bps;
   // MODE_DKV: key blocks >= n_train are invalid (skipped).  With blk = w % bps a CTA (w = x + 148 k) would see
@@ -101,11 +101,15 @@ __device__ __forceinline__ Item decode_item(const Shape& s, const Meta& meta, in
   // none (1.33x imbalance, base) -- so the block index is rotated by the sequence index.
   it.blk = MODE == MODE_DKV ? (w % bps + rest) % bps : w % bps;
   it.h = rest % s.H;
-  const int bc = rest / s.H;
-  it.b = bc / s.C;
-  it.c = bc - it.b * s.C;
+  const int bc = rest / s.H;          // (masked: the virtual column, an index into the list of valid pairs)
+  if (cl.masked()) {
+    cl.pair(bc, it.b, it.c);
+  } else {
+    it.b = bc / s.C;
+    it.c = bc - it.b * s.C;
+  }
   it.n = meta.n(s, it.b);
-  it.valid = meta.cv(s, bc) && (MODE == MODE_DQ || it.blk * kTileRows < it.n);
+  it.valid = MODE == MODE_DQ || it.blk * kTileRows < it.n;
   it.chunks = ((MODE == MODE_DQ ? it.n : s.R) + kChunk - 1) / kChunk;
   return it;
 }
@@ -117,13 +121,14 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
                : "memory");
 }
 
-template <int DH, int MODE>
+template <int DH, int MODE, bool MASKED>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_constant__ CUtensorMap mapA2,
                    const __grid_constant__ CUtensorMap mapB1, const __grid_constant__ CUtensorMap mapB2,
                    const __grid_constant__ CUtensorMap mapO, Shape s, const float* __restrict__ LSE,
                    float* lse2_ws, float* D_ws, uint4* Drec_ws, __nv_bfloat16* __restrict__ out0,
-                   __nv_bfloat16* __restrict__ out1, int n_items, int blocks_per_seq, int Rp) {
+                   __nv_bfloat16* __restrict__ out1, const uint32_t* __restrict__ col_list, int n_items_all,
+                   int blocks_per_seq, int Rp) {
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE_A = Cfg::TILE_A, TILE_B = Cfg::TILE_B, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -147,6 +152,9 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
   __shared__ uint8_t s_colvalid[kMetaCells];
   Meta meta;
   meta.fill(s, s_ntrain, s_colvalid);
+  ColList<MASKED> cl;
+  cl.init(s, col_list);
+  const int n_items = MASKED ? cl.nv * s.H * blocks_per_seq : n_items_all;   // (unmasked: a kernel parameter, uniform)
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // provably warp-uniform
   if (warp == kScoreWarps + 1) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
@@ -199,7 +207,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       if (MODE == MODE_DQ) tma_prefetch_desc(&mapO);
       uint32_t t = 0, k = 0;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-        const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+        const Item it = decode_item<MODE, MASKED>(s, meta, cl, w, blocks_per_seq);
         if (!it.valid) continue;
         const uint32_t ab = k & 1, a_full = smem_u32(&bar_a_full[ab]);
         mbar_wait<true>(smem_u32(&bar_a_empty[ab]), ((k >> 1) & 1) ^ 1);
@@ -243,7 +251,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                    b_s_empty = smem_u32(&bar_s_empty[0]);
     uint32_t t = 0, k = 0, st = 0, ph = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+      const Item it = decode_item<MODE, MASKED>(s, meta, cl, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
       mbar_wait(b_a_full + 8 * ab, (k >> 1) & 1);
@@ -293,7 +301,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                    b_b_empty = smem_u32(&bar_b_empty[0]);
     uint32_t t = 0, k = 0, st = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+      const Item it = decode_item<MODE, MASKED>(s, meta, cl, w, blocks_per_seq);
       if (!it.valid) continue;
       mbar_wait(smem_u32(&bar_acc_free), (k & 1) ^ 1);
       for (int j = 0; j < it.chunks; ++j, ++t) {
@@ -322,7 +330,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
     const int sub = lane / CH, ch = lane % CH;
     uint32_t k = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+      const Item it = decode_item<MODE, MASKED>(s, meta, cl, w, blocks_per_seq);
       if (!it.valid) continue;
       const uint32_t ab = k & 1;
       const size_t seq = ((size_t)it.b * s.C + it.c) * s.H + it.h;
@@ -447,14 +455,37 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           }
         }
     };
+    // a6: the invalid columns (masked tables) are dealt to the CTAs like the items (dQ, or dK and dV, := +0); a CTA
+    // clears one invalid item after every item it walks, so the stores spread over the kernel
+    const int n_zero = MASKED ? cl.ni * s.H * blocks_per_seq : 0;
+    int wz = blockIdx.x;
+    auto zero_one = [&]() {
+      const int blk = wz % blocks_per_seq, seq = wz / blocks_per_seq, h = seq % s.H;
+      int b, cc;
+      cl.pair(cl.nv + seq / s.H, b, cc);
+      const int row = blk * kTileRows + r;
+      if (row < s.R && c == 0) {
+        const size_t cell = (((size_t)b * s.R + row) * s.C + cc) * d + (size_t)h * DH;
+        if (MODE == MODE_DQ) {
+#pragma unroll
+          for (int k = 0; k < DH / 16; ++k) stg_v4(out0 + cell + g * (DH / 2) + 8 * k, make_uint4(0, 0, 0, 0));
+        } else {
+          __nv_bfloat16* dst = (g == 0 ? out0 : out1) + cell;
+#pragma unroll
+          for (int k = 0; k < DH / 8; ++k) stg_v4(dst + 8 * k, make_uint4(0, 0, 0, 0));
+        }
+      }
+      wz += gridDim.x;
+    };
     bool pend = false;
     size_t p_cell = 0;
     int p_row = 0, p_n = 0;
     uint32_t p_par = 0;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-      const Item it = decode_item<MODE>(s, meta, w, blocks_per_seq);
+      const Item it = decode_item<MODE, MASKED>(s, meta, cl, w, blocks_per_seq);
       const int row = it.blk * kTileRows + r;
       const size_t cell = (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
+      if (MASKED && wz < n_zero) zero_one();
       if (!it.valid) {
         // invalid column, or (MODE_DKV) a key block entirely beyond the train rows: zeros
         if (row < s.R && c == 0) {
@@ -569,6 +600,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       tbase += chunks;
     }
     if (pend) epilogue(p_cell, p_row, p_n, p_par);
+    while (MASKED && wz < n_zero) zero_one();   // (what is left of the invalid columns)
   }
   tc_fence_before();
   __syncthreads();
@@ -589,23 +621,27 @@ cudaError_t launch_bwd(const Shape& s, const void* Q, const void* K, const void*
                   map(&k128, K, kTileRows) && map(&v128, V, kTileRows) && map(&q64, Q, kChunk) &&
                   map(&g64, dO, kChunk) && map(&k64, K, kChunk) && map(&v64, V, kChunk);
   if (!ok) return cudaErrorInvalidValue;
-  auto kq = item_bwd_tc_kernel<DH, MODE_DQ>;
-  auto kkv = item_bwd_tc_kernel<DH, MODE_DKV>;
-  static SmemAttr attr_q, attr_kv;
-  cudaError_t e = attr_q.ensure(kq, Cfg::SMEM, di->ordinal);
-  if (e == cudaSuccess) e = attr_kv.ensure(kkv, Cfg::SMEM, di->ordinal);
+  const bool masked = s.col_valid != nullptr;
+  auto kq = masked ? item_bwd_tc_kernel<DH, MODE_DQ, true> : item_bwd_tc_kernel<DH, MODE_DQ, false>;
+  auto kkv = masked ? item_bwd_tc_kernel<DH, MODE_DKV, true> : item_bwd_tc_kernel<DH, MODE_DKV, false>;
+  static SmemAttr attr_q[2], attr_kv[2];
+  cudaError_t e = attr_q[masked].ensure(kq, Cfg::SMEM, di->ordinal);
+  if (e == cudaSuccess) e = attr_kv[masked].ensure(kkv, Cfg::SMEM, di->ordinal);
   if (e != cudaSuccess) return e;
   const int Rp = item_bwd_padded_rows(s);
   float* lse2_ws = ws;
   float* D_ws = ws + (size_t)s.B * s.C * s.H * Rp;            // fp32 D per row (dh = 64) ...
   uint4* Drec_ws = reinterpret_cast<uint4*>(D_ws);            // ... or one 32-byte D record per row (dh <= 32)
   const int bps = (s.R + kTileRows - 1) / kTileRows;
-  const long long n_items = (long long)s.B * s.C * s.H * bps;
+  const long long n_items = (long long)s.B * s.C * s.H * bps;   // (upper bound: masked tables walk the valid pairs only)
   const int grid = (int)std::min<long long>(n_items, di->num_sms);
+  // a0: the column list sits behind the row statistics in the workspace
+  const size_t stat_bytes = (size_t)s.B * s.C * s.H * Rp * (sizeof(float) + (s.dh <= 32 ? 32 : sizeof(float)));
+  const uint32_t* list = item_build_list(s, reinterpret_cast<char*>(ws) + stat_bytes, stream);
   kq<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(q128, g128, k64, v64, o128, s, LSE, lse2_ws, D_ws, Drec_ws,
-                                               (__nv_bfloat16*)dQ, nullptr, (int)n_items, bps, Rp);
+                                               (__nv_bfloat16*)dQ, nullptr, list, (int)n_items, bps, Rp);
   kkv<<<grid, kBwdThreads, Cfg::SMEM, stream>>>(k128, v128, q64, g64, o128, s, LSE, lse2_ws, D_ws, Drec_ws,
-                                                (__nv_bfloat16*)dV, (__nv_bfloat16*)dK, (int)n_items, bps, Rp);
+                                                (__nv_bfloat16*)dV, (__nv_bfloat16*)dK, list, (int)n_items, bps, Rp);
   count_launch(2);
   return cudaGetLastError();
 }
@@ -619,7 +655,7 @@ int item_bwd_padded_rows(const Shape& s) { return (s.R + kChunk - 1) / kChunk * 
 size_t item_bwd_workspace_bytes(const Shape& s) {
   // per query row: -LSE log2(e) as f32, and D as f32 (dh = 64) or as a 32-byte operand record (dh <= 32, BwdCfg::FOLD)
   const size_t per_row = sizeof(float) + (s.dh <= 32 ? 32 : sizeof(float));
-  return (size_t)s.B * s.C * s.H * item_bwd_padded_rows(s) * per_row;
+  return (size_t)s.B * s.C * s.H * item_bwd_padded_rows(s) * per_row + item_list_bytes(s);
 }
 
 cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,

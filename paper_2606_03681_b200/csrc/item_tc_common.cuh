@@ -13,6 +13,40 @@ constexpr float kRescaleLog2 = 8.f;  // lazy-rescale threshold of the online sof
 
 __device__ __forceinline__ int clamp_n(const Shape& s, int b) { return max(1, min(__ldg(s.n_train + b), s.R)); }
 
+// a0 for masked tables: the compacted list of (b, c) pairs, built by item_prep_kernel into the workspace:
+//   counts[0] = NV valid pairs;  list[0, NV) = the valid pairs ascending, list[NV, B*C) = the invalid ones, each
+//   packed as b << 16 | c.
+// The kernels walk virtual columns v in [0, NV) instead of all B*C columns and skipping the invalid ones: a skipped
+// item costs nothing, so the static walk dealt uneven numbers of real items to the CTAs (feature_heavy: 40 % of the
+// columns invalid, per-SM busy time max / avg = 1.08-1.11, profiles/r02_attention.md).  The zero-fill of the invalid
+// columns (a6) is a second, equally dealt walk over list[NV, B*C) after the main loop.  list == nullptr (no mask):
+// every column is valid and v is the real column index.
+// MASKED is a template parameter of the kernels: the unmasked instantiations carry none of this (the forward's
+// softmax loop lost 15 % at base when the list pointer was a run-time member of its walker).
+template <bool MASKED>
+struct ColList {
+  const uint32_t* list;
+  int nv, ni;
+  __device__ __forceinline__ void init(const Shape& s, const uint32_t* l) {
+    list = nullptr;
+    nv = s.B * s.C;
+    ni = 0;
+    if (MASKED) {
+      nv = (int)__ldg(l);          // counts[0] sits in front of the list
+      ni = s.B * s.C - nv;
+      list = l + 4;
+    }
+  }
+  static __device__ __forceinline__ constexpr bool masked() { return MASKED; }
+  // returns false only for the (never written) entry 0xffffffff: B, C <= 65535 keep every real pair below it
+  __device__ __forceinline__ bool pair(int v, int& b, int& c) const {
+    const uint32_t e = __ldg(list + v);
+    b = (int)(e >> 16);
+    c = (int)(e & 0xffffu);
+    return e != 0xffffffffu;
+  }
+};
+
 // Per-table metadata (clamped n_train, column validity) staged in shared memory at kernel start when it fits:
 // every role decodes every work item, and the two dependent global loads behind each decode were exposed at
 // every item boundary (items are only 12-16 chunks long at base).  Larger problems read global memory.  Used by
@@ -52,8 +86,10 @@ struct ItemCoord {
   int w, blk, h, c, b, seqmod;
   int s_blk, s_h, s_c, s_b, s_seqmod;   // per-step increments (step = gridDim.x items)
   int bps, H, C;
-  __device__ __forceinline__ void init(const Shape& s, int bps_) {
-    bps = bps_; H = s.H; C = s.C;
+  // `cols`: number of columns walked -- s.C per table, or (masked) the NV valid pairs as one virtual table, in which
+  // case c is the virtual column and b stays 0
+  __device__ __forceinline__ void init(const Shape& s, int bps_, int cols = 0) {
+    bps = bps_; H = s.H; C = cols > 0 ? cols : s.C;
     w = blockIdx.x;
     blk = w % bps;
     const int seq = w / bps;
@@ -93,6 +129,7 @@ struct ItemCoord {
   }
 };
 
+template <bool MASKED>
 struct Walker {
   ItemCoord ic;
   int j, tiles, n, b, c, h, blk;
@@ -101,10 +138,16 @@ struct Walker {
   int n_items, chunk;        // items in the launch, rows per inner tile
   bool over_keys;            // inner axis = key rows [0, n) (fwd, dQ); else query rows [0, R) (dK/dV)
 
+  ColList<MASKED> cl;
   __device__ __forceinline__ void decode(const Shape& s, bool& valid) {
     blk = ic.blk; h = ic.h; b = ic.b; c = ic.c;
+    bool listed = true;
+    if (cl.masked()) listed = cl.pair(ic.c, b, c);
     n = clamp_n(s, b);
-    valid = (!s.col_valid || __ldg(s.col_valid + ic.bc()) != 0) && (over_keys || blk * kTileRows < n);
+    // (both instantiations keep a run-time validity test that is never false -- the unmasked one the mask test of
+    // the earlier builds, the masked one the list entry's -- because without the branch it guards ptxas schedules
+    // the forward's softmax loop 7 % slower: 0.574 against 0.535 ms at base, measured A/B on one box)
+    valid = (MASKED ? listed : (!s.col_valid || __ldg(s.col_valid + ic.bc()) != 0)) && (over_keys || blk * kTileRows < n);
     tiles = ((over_keys ? n : s.R) + chunk - 1) / chunk;
   }
   __device__ __forceinline__ void seek(const Shape& s) {
@@ -120,9 +163,10 @@ struct Walker {
       ic.next();
     }
   }
-  __device__ __forceinline__ void init(const Shape& s, int n_items_, int bps_, int chunk_, bool over_keys_) {
-    n_items = n_items_; chunk = chunk_; over_keys = over_keys_;
-    ic.init(s, bps_);
+  __device__ __forceinline__ void init(const Shape& s, const ColList<MASKED>& cl_, int bps_, int chunk_, bool over_keys_) {
+    cl = cl_; chunk = chunk_; over_keys = over_keys_;
+    n_items = cl.nv * s.H * bps_;
+    ic.init(s, bps_, cl.masked() ? max(cl.nv, 1) : 0);
     k = 0; t = 0;
     seek(s);
   }
@@ -158,4 +202,10 @@ __device__ __forceinline__ void setmaxnreg_dec() {
 }
 
 }  // namespace itc
+
+// (item_tc_fwd.cu) bytes of the column list in a workspace, and the launch of the a0 prep kernel that fills it;
+// returns the device pointer the kernels take (nullptr when the call has no mask)
+size_t item_list_bytes(const Shape& s);
+const uint32_t* item_build_list(const Shape& s, void* list_ws, cudaStream_t stream);
+
 }  // namespace tabattn

@@ -45,11 +45,12 @@ struct FwdCfg {
 
 constexpr int kFwdThreads = 384;
 
-template <int DH>
+template <int DH, bool MASKED>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                    const __grid_constant__ CUtensorMap mapV, Shape s, __nv_bfloat16* __restrict__ O,
-                   float* __restrict__ LSE, int n_items, int blocks_per_seq, int q_row0, int q_row1) {
+                   float* __restrict__ LSE, const uint32_t* __restrict__ col_list, int n_items_all,
+                   int blocks_per_seq, int q_row0, int q_row1) {
   using Cfg = FwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE = Cfg::TILE, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -62,6 +63,10 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
   __shared__ uint32_t tmem_slot;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // provably warp-uniform
+  ColList<MASKED> cl;
+  cl.init(s, col_list);
+  // (unmasked: the host's count, a kernel parameter, keeps the issuing warps' loop bounds in uniform registers)
+  const int n_items = MASKED ? cl.nv * s.H * blocks_per_seq : n_items_all;
   if (warp == 10) tmem_alloc(smem_u32(&tmem_slot), Cfg::COLS);
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
@@ -94,8 +99,8 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         tma_prefetch_desc(&mapQ);
         tma_prefetch_desc(&mapK);
         tma_prefetch_desc(&mapV);
-        Walker wk;
-        for (wk.init(s, n_items, blocks_per_seq, kTileRows, true); wk.ok; wk.next(s)) {
+        Walker<MASKED> wk;
+        for (wk.init(s, cl, blocks_per_seq, kTileRows, true); wk.ok; wk.next(s)) {
           if (wk.j == 0) {
             const int qb = wk.k & 1;
             mbar_wait<true>(smem_u32(&bar_q_empty[qb]), ((wk.k >> 1) & 1) ^ 1);
@@ -128,15 +133,14 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       uint32_t st = 0, ph = 0, par = 0, j = 0, tiles = 0, k = 0;
       int n = 0;
       ItemCoord ic;
-      ic.init(s, blocks_per_seq);
+      ic.init(s, blocks_per_seq, cl.masked() ? max(cl.nv, 1) : 0);
       auto seek = [&]() {
-        for (; ic.w < n_items; ic.next()) {
-          if (s.col_valid && __ldg(s.col_valid + ic.bc()) == 0) continue;
-          n = clamp_n(s, ic.b);
-          tiles = (uint32_t)(n + kTileRows - 1) / kTileRows;
-          return true;
-        }
-        return false;
+        if (ic.w >= n_items) return false;
+        int rb = ic.b, rc = ic.c;
+        if (cl.masked()) cl.pair(ic.c, rb, rc);
+        n = clamp_n(s, rb);
+        tiles = (uint32_t)(n + kTileRows - 1) / kTileRows;
+        return true;
       };
       bool ok = seek();
       if (warp == 9) {
@@ -226,16 +230,33 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const float c2 = s.scale * kLog2e;
     const int d = s.H * DH;
     uint32_t g = 0;  // tiles processed by this CTA so far
-    Walker it;
-    it.n_items = n_items; it.chunk = kTileRows; it.over_keys = true;
-    it.ic.init(s, blocks_per_seq);
+    // a6: the invalid columns (masked tables) are dealt to the CTAs like the items (O := +0, LSE := 0); a CTA clears
+    // one invalid item after every item it computes, so the stores spread over the kernel instead of forming a tail
+    const int n_zero = MASKED ? cl.ni * s.H * blocks_per_seq : 0;
+    int wz = blockIdx.x;
+    auto zero_one = [&]() {
+      const int blk = wz % blocks_per_seq, seq = wz / blocks_per_seq, h = seq % s.H;
+      int b, c;
+      cl.pair(cl.nv + seq / s.H, b, c);
+      const int row = q_row0 + blk * 2 * kTileRows + t * kTileRows + r;
+      if (row < q_row1) {
+        __nv_bfloat16* oz = O + (((size_t)b * s.R + row) * s.C + c) * d + (size_t)h * DH;
+#pragma unroll
+        for (int k = 0; k < DH / 8; ++k) stg_v4(oz + 8 * k, make_uint4(0, 0, 0, 0));
+        if (LSE) LSE[(((size_t)b * s.C + c) * s.H + h) * s.R + row] = 0.f;
+      }
+      wz += gridDim.x;
+    };
+    Walker<MASKED> it;
+    it.cl = cl; it.n_items = n_items; it.chunk = kTileRows; it.over_keys = true;
+    it.ic.init(s, blocks_per_seq, cl.masked() ? max(cl.nv, 1) : 0);
     for (; it.ic.w < n_items; it.ic.next()) {
       bool valid;
       it.decode(s, valid);
       const int row = q_row0 + it.blk * 2 * kTileRows + t * kTileRows + r;
       __nv_bfloat16* orow = O + (((size_t)it.b * s.R + row) * s.C + it.c) * d + (size_t)it.h * DH;
       float* lse = LSE + (((size_t)it.b * s.C + it.c) * s.H + it.h) * s.R + row;
-      if (!valid) {
+      if (!valid) {   // (never taken: see Walker::decode)
         if (row < q_row1) {
 #pragma unroll
           for (int k = 0; k < DH / 8; ++k) stg_v4(orow + 8 * k, make_uint4(0, 0, 0, 0));
@@ -334,7 +355,9 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
         if (LSE) *lse = (m + log2f(l)) * kLn2;
       }
+      if (MASKED && wz < n_zero) zero_one();
     }
+    while (MASKED && wz < n_zero) zero_one();   // (what is left of the invalid columns)
   }
   tc_fence_before();
   __syncthreads();
@@ -343,7 +366,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 
 template <int DH>
 cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                       int q_row0, int q_row1, cudaStream_t stream) {
+                       int q_row0, int q_row1, void* ws, cudaStream_t stream) {
   using Cfg = FwdCfg<DH>;
   const DeviceInfo* di = current_device();
   if (!di) return cudaErrorInvalidDevice;
@@ -352,28 +375,83 @@ cudaError_t launch_fwd(const Shape& s, const void* Q, const void* K, const void*
       !get_tensor_map(&mk, 0, K, s.B, s.R, s.C, s.H, DH, kTileRows, 1) ||
       !get_tensor_map(&mv, 0, V, s.B, s.R, s.C, s.H, DH, kTileRows, 1))
     return cudaErrorInvalidValue;
-  auto kern = item_fwd_tc_kernel<DH>;
-  static SmemAttr attr;
-  cudaError_t e = attr.ensure(kern, Cfg::SMEM, di->ordinal);
+  const uint32_t* list = item_build_list(s, ws, stream);   // (a0 prep kernel for masked tables)
+  auto kern = list ? item_fwd_tc_kernel<DH, true> : item_fwd_tc_kernel<DH, false>;
+  static SmemAttr attr_m, attr_u;
+  cudaError_t e = (list ? attr_m : attr_u).ensure(kern, Cfg::SMEM, di->ordinal);
   if (e != cudaSuccess) return e;
   // query rows [q_row0, q_row1) of every sequence (the training forward passes [0, R)); keys are always [0, n_train)
   const int bps = (q_row1 - q_row0 + 2 * kTileRows - 1) / (2 * kTileRows);
   const long long n_items = (long long)s.B * s.C * s.H * bps;
   const int grid = (int)std::min<long long>(n_items, di->num_sms);
-  kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, (int)n_items, bps, q_row0,
-                                                 q_row1);
+  kern<<<grid, kFwdThreads, Cfg::SMEM, stream>>>(mq, mk, mv, s, (__nv_bfloat16*)O, LSE, list, (int)n_items, bps, q_row0, q_row1);
   count_launch();
   return cudaGetLastError();
 }
 
 }  // namespace
 
+// ---- a0 prep (masked tables): the compacted (b, c) list of item_tc_common.cuh ---------------------------------
+__global__ void __launch_bounds__(256) item_prep_kernel(Shape s, uint32_t* __restrict__ out) {
+  __shared__ int warp_cnt[8];
+  __shared__ int base_s, nv_s;
+  const int cells = s.B * s.C, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint32_t* list = out + 4;
+  // pass 1: NV
+  int cnt = 0;
+  for (int i = threadIdx.x; i < cells; i += 256) cnt += __ldg(s.col_valid + i) != 0;
+  for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+  if (lane == 0) warp_cnt[warp] = cnt;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int t = 0;
+    for (int w = 0; w < 8; ++w) t += warp_cnt[w];
+    nv_s = t;
+    base_s = 0;
+    out[0] = (uint32_t)t;
+  }
+  __syncthreads();
+  const int nv = nv_s;
+  // pass 2: valid pairs ascending into [0, NV), invalid ones ascending into [NV, cells)
+  for (int i0 = 0; i0 < cells; i0 += 256) {
+    const int i = i0 + threadIdx.x;
+    const bool in = i < cells, v = in && __ldg(s.col_valid + i) != 0;
+    const uint32_t m = __ballot_sync(0xffffffffu, v);
+    if (lane == 0) warp_cnt[warp] = __popc(m);
+    __syncthreads();
+    int before = base_s;                       // valid pairs before this 256-chunk
+    for (int w = 0; w < warp; ++w) before += warp_cnt[w];
+    before += __popc(m & ((1u << lane) - 1u));
+    if (in) {
+      const int b = i / s.C, c = i - b * s.C;
+      list[v ? before : nv + (i - before)] = ((uint32_t)b << 16) | (uint32_t)c;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int t = 0;
+      for (int w = 0; w < 8; ++w) t += warp_cnt[w];
+      base_s += t;
+    }
+    __syncthreads();
+  }
+}
+
+size_t item_list_bytes(const Shape& s) { return ((size_t)s.B * s.C + 4) * sizeof(uint32_t); }
+size_t item_fwd_workspace_bytes(const Shape& s) { return item_list_bytes(s); }
+
+const uint32_t* item_build_list(const Shape& s, void* list_ws, cudaStream_t stream) {
+  if (!s.col_valid || !list_ws) return nullptr;
+  item_prep_kernel<<<1, 256, 0, stream>>>(s, static_cast<uint32_t*>(list_ws));
+  count_launch();
+  return static_cast<const uint32_t*>(list_ws);
+}
+
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                            int q_row0, int q_row1, cudaStream_t stream) {
+                            int q_row0, int q_row1, void* ws, cudaStream_t stream) {
   switch (s.dh) {
-    case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
-    case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
-    case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, q_row0, q_row1, stream);
+    case 16: return launch_fwd<16>(s, Q, K, V, O, LSE, q_row0, q_row1, ws, stream);
+    case 32: return launch_fwd<32>(s, Q, K, V, O, LSE, q_row0, q_row1, ws, stream);
+    case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, q_row0, q_row1, ws, stream);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -26,8 +26,10 @@ size_t feature_workspace_bytes(const Shape& s);   // masked calls: per-table geo
 // D = rowsum(dO o O) as f32 (dh = 64) or as a 32-byte MMA operand record (dh <= 32); written by the dQ pass and
 // read by the dK/dV pass.  The forward needs none.
 // query rows [q_row0, q_row1) of every sequence; LSE may be NULL (inference)
+// ws: item_fwd_workspace_bytes(s) bytes, only touched when a column mask is given (the a0 column list)
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
-                            int q_row0, int q_row1, cudaStream_t stream);
+                            int q_row0, int q_row1, void* ws, cudaStream_t stream);
+size_t item_fwd_workspace_bytes(const Shape& s);
 cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
                             const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
                             cudaStream_t stream);

@@ -52,7 +52,8 @@ def test_workspace_bytes(tab):
     # feature calls: per-table geometry for masked tables (a0), a few KB
     assert 32 * (16 + 128) <= tab.workspace_bytes(s, tab.OP_FEATURE_FWD) <= 32 * 256
     assert tab.workspace_bytes(s, tab.OP_FEATURE_BWD) == tab.workspace_bytes(s, tab.OP_FEATURE_FWD)
-    assert tab.workspace_bytes(s, tab.OP_ITEM_FWD) == 0
+    # item forward: the a0 column list of masked calls, 4 bytes per (b, c) pair
+    assert 32 * 11 * 4 <= tab.workspace_bytes(s, tab.OP_ITEM_FWD) <= 32 * 11 * 4 + 64
     # D = rowsum(dO o O) as f32 [B,C,H,R] must fit
     assert tab.workspace_bytes(s, tab.OP_ITEM_BWD) >= 32 * 11 * 6 * 1024 * 4
     bad = tab.TabattnShape(32, 1024, 11, 6, 48, None, None, None, 0.0)
