@@ -83,7 +83,7 @@ struct BwdCfg {
   static constexpr int ACC0 = 384, ACC1 = 384 + DH, COLS = 512;
   static_assert(ACC1 + DH <= COLS, "TMEM budget");
   // pairs of every 8 whose exponential runs on the FMA pipe (exp2_poly2, common.cuh) instead of the MUFU
-  static constexpr int POLY_OF_8 = DH >= 64 ? 0 : 2;
+  static constexpr int POLY_OF_8 = DH >= 64 ? 0 : 1;
 };
 
 // One work item = (table b, column c, head h, 128-row block blk) of the stationary axis.
