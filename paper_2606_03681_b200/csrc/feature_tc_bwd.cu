@@ -486,6 +486,8 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       tc_fence_after();
       const size_t off = ((size_t)(grow0 + rl) * s.C + my_col) * d2 + (size_t)x.h * ROWB;
       const uint64_t sc = f2pack(s.scale, s.scale);
+      QuadRows qr;
+      if constexpr (DH >= 32) qr.init(off, live, lane);
 #pragma unroll
       for (int w = 0; w < 3; ++w) {
         uint32_t acc[DH];
@@ -495,20 +497,31 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           __syncwarp();
           if (lane == 0) mbar_arrive(b_acc_free);
         }
-        if (live) {
-          unsigned char* dst = (w == 0 ? dQ : (w == 1 ? dK : dV)) + off;
+        unsigned char* dst = w == 0 ? dQ : (w == 1 ? dK : dV);
+        uint4 u[DH / 8];
 #pragma unroll
-          for (int q = 0; q < DH / 8; ++q) {
-            uint4 u;
-            uint32_t* up = &u.x;
+        for (int q = 0; q < DH / 8; ++q) {
+          uint32_t* up = &u[q].x;
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              float a = __uint_as_float(acc[8 * q + 2 * e]), b = __uint_as_float(acc[8 * q + 2 * e + 1]);
-              if (w < 2) f2unpack(mul2(f2pack(a, b), sc), a, b);
-              up[e] = pack_bf16(a, b);
-            }
-            stg_v4(dst + 16 * q, u);
+          for (int e = 0; e < 4; ++e) {
+            float a = __uint_as_float(acc[8 * q + 2 * e]), b = __uint_as_float(acc[8 * q + 2 * e + 1]);
+            if (w < 2) f2unpack(mul2(f2pack(a, b), sc), a, b);
+            up[e] = pack_bf16(a, b);
           }
+        }
+        if constexpr (DH >= 32) {
+          // a quad of lanes stores one 64-byte group of a row per instruction (quad_transpose, feature_tc.cuh)
+#pragma unroll
+          for (int gq = 0; gq < DH / 32; ++gq) {
+            uint4 t4[4] = {u[4 * gq], u[4 * gq + 1], u[4 * gq + 2], u[4 * gq + 3]};
+            quad_transpose(t4, lane);
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4)
+              if (qr.live[k4]) stg_v4(dst + qr.off[k4] + 64 * gq, t4[k4]);
+          }
+        } else if (live) {
+#pragma unroll
+          for (int q = 0; q < DH / 8; ++q) stg_v4(dst + off + 16 * q, u[q]);
         }
       }
     }
