@@ -393,19 +393,34 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           bulk_commit();
         }
         ++n_store;
-      } else if (pd_live) {
-        unsigned char* dst = O + ((size_t)pd_row * s.C + pd_col) * d2 + (size_t)pd_h * ROWB;
+      } else {
+        // gathered columns: a quad of lanes stores one 64-byte group of a row per instruction (quad_transpose)
+        const size_t off = ((size_t)pd_row * s.C + pd_col) * d2 + (size_t)pd_h * ROWB;
+        uint4 u[DH / 8];
 #pragma unroll
         for (int q = 0; q < DH / 8; ++q) {
-          uint4 u;
-          uint32_t* up = &u.x;
+          uint32_t* up = &u[q].x;
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             float a, b;
             f2unpack(mul2(f2pack(__uint_as_float(o[8 * q + 2 * e]), __uint_as_float(o[8 * q + 2 * e + 1])), iv), a, b);
             up[e] = pack_bf16(a, b);
           }
-          stg_v4(dst + 16 * q, u);
+        }
+        if constexpr (DH >= 32) {
+          QuadRows qr;
+          qr.init(off, pd_live, lane);
+#pragma unroll
+          for (int gq = 0; gq < DH / 32; ++gq) {
+            uint4 t4[4] = {u[4 * gq], u[4 * gq + 1], u[4 * gq + 2], u[4 * gq + 3]};
+            quad_transpose(t4, lane);
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4)
+              if (qr.live[k4]) stg_v4(O + qr.off[k4] + 64 * gq, t4[k4]);
+          }
+        } else if (pd_live) {
+#pragma unroll
+          for (int q = 0; q < DH / 8; ++q) stg_v4(O + off + 16 * q, u[q]);
         }
       }
     };
