@@ -429,7 +429,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         };
         // The single P/dS buffer is the serial section of the kernel (a tile holds it from its first store to
         // the completion of its accumulation MMAs), so everything that can be computed before the tile's turn
-        // is: for W <= 64 the dS chunks wait in registers and the turn only covers the stores
+        // is: the dS chunks wait in registers (W <= 64) or in TMEM (W = 128) and the turn only covers the stores
         // (profiles/r02_attention.md: the turn wait was 20 % of the softmax warps' samples at base).
         constexpr bool PRE = NCH <= 2;
         uint32_t dsr[PRE ? 16 * NCH : 16];
@@ -446,6 +446,18 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
 #pragma unroll
             for (int q = 0; q < 16; ++q) dsr[16 * c + q] = ds[q];
           }
+        } else {
+          // W = 128: the packed dS chunks are parked in TMEM, over the first half of the dP chunk they came from
+#pragma unroll
+          for (int c = 0; c < NCH; ++c) {
+            uint32_t pk[16], ds[16];
+            p_chunk(c, pk);
+            tmem_ld32(tS + colbase + 32 * c, dr);
+            tmem_wait_ld();
+            ds_chunk(pk, ds);
+            tmem_st16(tS + colbase + 32 * c, ds);
+          }
+          tmem_wait_st();
         }
         // this tile's turn on the P/dS buffer
         if (!first_tile) mbar_wait(b_turn, (g == 0 ? k - 1 : k) & 1);
@@ -466,9 +478,8 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
 #pragma unroll
             for (int q = 0; q < 16; ++q) ds[q] = dsr[16 * c + q];
           } else {
-            tmem_ld32(tS + colbase + 32 * c, dr);
+            tmem_ld16(tS + colbase + 32 * c, ds);
             tmem_wait_ld();
-            ds_chunk(pk, ds);
           }
           store_chunk(c, pk, ds);
         }
