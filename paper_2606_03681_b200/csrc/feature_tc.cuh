@@ -261,43 +261,8 @@ struct Gather {
   }
 };
 
-// 4 x 4 transpose of 16-byte chunks among the four lanes of a quad: on return lane i of the quad holds in a[k] the
-// chunk i that lane k of the quad passed in.  It turns "every lane stores its own 64-byte row in four instructions"
-// (32 different lines per instruction) into "a quad stores one row per instruction" (8 lines per instruction): the
-// per-thread row stores of the backward were 1,536 line requests per tile and kept the LSU busy for the whole tile
-// period, which also delayed the shared-memory stores of the serial P/dS section (timeline in profiles/r02_attention.md).
-__device__ __forceinline__ void quad_transpose(uint4 (&a)[4], int lane) {
-#pragma unroll
-  for (int st = 0; st < 2; ++st) {
-    const int m = 1 << st;
-    const bool up = (lane & m) != 0;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      if (c & m) continue;
-      uint4 send = up ? a[c] : a[c | m];
-      send.x = __shfl_xor_sync(0xffffffffu, send.x, m);
-      send.y = __shfl_xor_sync(0xffffffffu, send.y, m);
-      send.z = __shfl_xor_sync(0xffffffffu, send.z, m);
-      send.w = __shfl_xor_sync(0xffffffffu, send.w, m);
-      if (up) a[c] = send; else a[c | m] = send;
-    }
-  }
-}
-
-// Offsets and liveness of the four rows of this lane's quad, as seen by the lane that stores chunk (lane & 3) of them.
-struct QuadRows {
-  size_t off[4];
-  bool live[4];
-  __device__ __forceinline__ void init(size_t my_off, bool my_live, int lane) {
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int src = (lane & ~3) + k;
-      const unsigned long long o = __shfl_sync(0xffffffffu, (unsigned long long)my_off, src);
-      off[k] = (size_t)o + (size_t)(lane & 3) * 16;
-      live[k] = __shfl_sync(0xffffffffu, (int)my_live, src) != 0;
-    }
-  }
-};
+using ::tabattn::quad_transpose;
+using ::tabattn::QuadRows;
 
 template <int N>
 __device__ __forceinline__ void setmaxnreg_inc() {

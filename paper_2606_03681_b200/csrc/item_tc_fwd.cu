@@ -344,7 +344,31 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       uint32_t o[DH];
       tmem_ld_cols<DH>(tO, o);
       tc_fence_before();
-      if (row < q_row1) {
+      if constexpr (DH >= 64) {
+        // a quad of lanes stores one 64-byte group of a row per instruction (four times fewer line requests than
+        // every lane storing its own row in DH / 8 instructions; measured +2 % at dh = 64, -2 % at dh = 32)
+        const float inv = 1.f / l;
+        uint4 u[DH / 8];
+#pragma unroll
+        for (int k = 0; k < DH / 8; ++k) {
+          float f[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(o[8 * k + e]) * inv;
+          u[k] = pack8(f);
+        }
+        const bool live = row < q_row1;
+        QuadRows qr;
+        qr.init(reinterpret_cast<size_t>(orow), live, lane);
+#pragma unroll
+        for (int gq = 0; gq < DH / 32; ++gq) {
+          uint4 t4[4] = {u[4 * gq], u[4 * gq + 1], u[4 * gq + 2], u[4 * gq + 3]};
+          quad_transpose(t4, lane);
+#pragma unroll
+          for (int k4 = 0; k4 < 4; ++k4)
+            if (qr.live[k4]) stg_v4(reinterpret_cast<void*>(qr.off[k4] + 64 * gq), t4[k4]);
+        }
+        if (live && LSE) *lse = (m + log2f(l)) * kLn2;
+      } else if (row < q_row1) {
         const float inv = 1.f / l;
 #pragma unroll
         for (int k = 0; k < DH / 8; ++k) {
