@@ -27,6 +27,21 @@
 
 namespace tabattn {
 
+// Timeline instrumentation (only with -DTABATTN_TRACE, `TABATTN_TRACE=1 python -m paper_2606_03681_b200.build`; the
+// shipped library has none of it): clock64() stamps of CTA 0's first 64 tiles, event e of tile n at trace[16 n + e].
+// paper_2606_03681_b200/trace_feature_bwd.py prints them; profiles/r02_attention.md has the reading that found the
+// LSU jam of the per-thread row stores.
+#ifdef TABATTN_TRACE
+__device__ long long* g_trace = nullptr;
+extern "C" __attribute__((visibility("default"))) void tabattn_debug_set_trace(long long* p) {
+  cudaMemcpyToSymbol(g_trace, &p, sizeof(p));
+}
+#define TR(ev, tile) \
+  do { if (blockIdx.x == 0 && (tile) < 64 && g_trace) g_trace[(tile) * 16 + (ev)] = clock64(); } while (0)
+#else
+#define TR(ev, tile) do { } while (0)
+#endif
+
 namespace {
 
 using namespace tc;
@@ -134,6 +149,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
             const uint32_t st = n % ST, full = smem_u32(&bar_full[st]), dst = sStage + st * STAGE;
             mbar_wait<true>(smem_u32(&bar_empty[st]), ((n / ST) & 1) ^ 1);
             mbar_arrive_expect_tx(full, STAGE);
+            TR(0, n);                                     // TMA issued
             tma_load_4d(dst, &mapQ, full, 0, x.h, 0, x.row0);
             tma_load_4d(dst + TILE, &mapK, full, 0, x.h, 0, x.row0);
             tma_load_4d(dst + 2 * TILE, &mapV, full, 0, x.h, 0, x.row0);
@@ -247,6 +263,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           last_bar = smem_u32(&bar_s_full[g]);
           last_par = k & 1;
           tc_commit_e(last_bar);
+          if (lane == 0) TR(1, n);                      // S MMAs issued
         } else {
           mbar_wait(smem_u32(&bar_full[st]), (n / ST) & 1);
           mbar_wait(smem_u32(&bar_s_taken[g]), k & 1);                     // every thread has read its S window
@@ -254,6 +271,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
 #pragma unroll
           for (int kk = 0; kk < DH / 16; ++kk) mma_ss_e(tS, ad + 2 * kk, bd + 2 * kk, idS, kk > 0);
           tc_commit_e(smem_u32(&bar_dp_full[g]));
+          if (lane == 0) TR(2, n);                      // dP MMAs issued
         }
         if (++g == NSETS) { g = 0; ++k; }
       }
@@ -280,6 +298,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       for (wk.init(p); wk.get(p, x); wk.next(p), ++n) {
         const uint32_t st = n % ST;
         mbar_wait(smem_u32(&bar_pds_full[g]), k & 1);
+        if (lane == 0) TR(3, n);                        // accumulation warp has P/dS
         tc_fence_after();
         const uint64_t so = (uint64_t)((st * STAGE) >> 4);
         const uint32_t tA = tmem + Cfg::SET * g;
@@ -293,6 +312,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         for (int kk = 0; kk < 8; ++kk)
           mma_ss_e(tA + 2 * DH, aPT + (uint64_t)(kk * (16 * 128 >> 4)), bG + so + kk * ROWB, idT, kk > 0);
         tc_commit_e(smem_u32(&bar_acc_full[g]));
+        if (lane == 0) TR(4, n);                        // accumulation MMAs issued
         tc_commit_e(smem_u32(&bar_empty[st]));
         if (++g == NSETS) { g = 0; ++k; }
       }
@@ -349,6 +369,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         uint32_t pp[16 * NREG];
         // ---- pass A: P = 2^(S c2 - LSE log2e), packed bf16 pairs
         mbar_wait(b_s_full, k & 1);
+        if (wq == 0 && lane == 0) TR(5, k * NSETS + g);   // softmax: S ready
         tc_fence_after();
         // -LSE log2(e) of the slot, staged with the tile (the stage's barrier completed before the S MMA was issued;
         // waiting on it here is what makes the producers' stores visible to this thread)
@@ -377,6 +398,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         if (NCH > NREG) tmem_wait_st();
         tc_fence_before();
         __syncwarp();
+        if (wq == 0 && lane == 0) TR(6, k * NSETS + g);   // pass A done
         if (lane == 0) mbar_arrive(b_s_taken);
         // packed P of chunk c (registers or the TMEM scratch)
         auto p_chunk = [&](int c, uint32_t (&pk)[16]) {
@@ -390,6 +412,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
         };
         // ---- pass B: D = sum P dP, then dS = P (dP - D), from the bf16-rounded P (the value the dV MMA uses)
         mbar_wait(b_dp_full, k & 1);
+        if (wq == 0 && lane == 0) TR(7, k * NSETS + g);   // dP ready
         tc_fence_after();
         uint64_t dacc = 0;
         uint32_t dr[32];
@@ -460,7 +483,9 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           tmem_wait_st();
         }
         // this tile's turn on the P/dS buffer
+        if (wq == 0 && lane == 0) TR(8, k * NSETS + g);   // pass B done, waiting for the turn
         if (!first_tile) mbar_wait(b_turn, (g == 0 ? k - 1 : k) & 1);
+        if (wq == 0 && lane == 0) TR(9, k * NSETS + g);   // turn acquired
         if (old_lg >= 0 && old_lg != x.lgCp) {
           // the rows were last written with another geometry: clear that window
           const int ocb = old_lg >= 5 ? (((32 * wq) >> old_lg) << old_lg) : 32 * wq;
@@ -490,10 +515,12 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       tc_fence_before();
       fence_proxy_async_smem();
       __syncwarp();
+      if (wq == 0 && lane == 0) TR(10, k * NSETS + g);    // P/dS stored and fenced
       if (lane == 0) mbar_arrive(b_pds_full);
 
       // ---- drain dQ | dK | dV
       mbar_wait(b_acc_full, k & 1);
+      if (wq == 0 && lane == 0) TR(11, k * NSETS + g);    // accumulators ready
       tc_fence_after();
       const size_t off = ((size_t)(grow0 + rl) * s.C + my_col) * d2 + (size_t)x.h * ROWB;
       const uint64_t sc = f2pack(s.scale, s.scale);
@@ -507,6 +534,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(b_acc_free);
+          if (wq == 0 && lane == 0) TR(12, k * NSETS + g);  // accumulators drained
         }
         unsigned char* dst = w == 0 ? dQ : (w == 1 ? dK : dV);
         uint4 u[DH / 8];
