@@ -5,6 +5,7 @@ arxiv/paper_2606_03681 speedruns (Fig. 3, L91, L277, L294): feature
 item-axis scaled-dot-product attention over a [B,R,C,H,dh] cell tensor.  The product is the
 C-ABI library declared in include/tabattn.h (csrc/); this package is its ctypes binding.
 """
+from . import binding
 from .binding import (TabattnError, TabattnShape, EXPORTS, LIB_PATH, lib, make_shape, status_string, version, launch_count,
                       workspace_bytes, tabattn_feature_fwd, tabattn_feature_bwd, tabattn_item_fwd,
                       tabattn_item_bwd, tabattn_feature_fwd_infer, tabattn_item_fwd_infer, OP_FEATURE_FWD, OP_FEATURE_BWD, OP_ITEM_FWD, OP_ITEM_BWD,

@@ -148,3 +148,40 @@ def test_product_never_imports_the_oracle():
         if fn.endswith((".py", ".c")):
             assert "paper_2606_03681_b200/csrc" in open(os.path.join(ROOT, "oracle", fn)).read() or \
                 "import paper_2606_03681_b200" not in open(os.path.join(ROOT, "oracle", fn)).read()
+
+
+def test_new_entry_points_reject_bad_arguments_without_a_device(tab):
+    """The evaluation and sub-block calls validate before they touch the device."""
+    L = tab.lib()
+    P = lambda i: ctypes.c_void_p(16 * (i + 1))
+    nt = (ctypes.c_int32 * 2)(3, 4)
+    s = tab.TabattnShape(2, 8, 4, 2, 32, 4096, ctypes.cast(nt, ctypes.c_void_p).value, None, 0.0)
+    # row range outside [0, R] or empty
+    for r0, r1 in ((-1, 4), (4, 4), (6, 2), (0, 9)):
+        assert L.tabattn_item_fwd_infer(ctypes.byref(s), P(0), P(1), P(2), P(3), r0, r1, None, 0, None) == tab.ERR_INVALID_ARG
+        assert L.tabattn_feature_fwd_infer(ctypes.byref(s), P(0), P(1), P(2), P(3), r0, r1, None, 0, None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_item_fwd_infer(ctypes.byref(s), P(0), P(1), P(2), P(0), 0, 8, None, 0, None) == tab.ERR_INVALID_ARG  # O over Q
+    # sub-blocks: e = H*dh must be a multiple of 64 (here 2 x 16 = 32), axis in {0, 1}, saved struct required
+    s32 = tab.TabattnShape(2, 8, 4, 2, 16, 4096, None, None, 0.0)
+    sv = tab.binding.TabattnAttnSaved(*[16 * (i + 20) for i in range(7)])
+    assert L.tabattn_attn_block_fwd(ctypes.byref(s32), 0, 1.0, 0.0, P(0), P(1), P(2), P(3), P(4), ctypes.byref(sv), None, 0,
+                                    None) == tab.ERR_UNSUPPORTED
+    s64 = tab.TabattnShape(2, 8, 4, 2, 32, 4096, None, None, 0.0)
+    assert L.tabattn_attn_block_fwd(ctypes.byref(s64), 2, 1.0, 0.0, P(0), P(1), P(2), P(3), P(4), ctypes.byref(sv), None, 0,
+                                    None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_attn_block_fwd(ctypes.byref(s64), 0, 1.0, 0.0, P(0), P(1), P(2), P(3), P(4), None, None, 0,
+                                    None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_attn_block_workspace_bytes(ctypes.byref(s64), 0, 1) > 2 * 8 * 4 * 64 * 2 * 5
+    assert L.tabattn_attn_block_workspace_bytes(ctypes.byref(s64), 3, 1) == 0
+    mv = tab.binding.TabattnMlpSaved(*[16 * (i + 30) for i in range(4)])
+    assert L.tabattn_mlp_fwd(100, 96, 128, 1.0, 0.0, P(0), P(1), P(2), P(3), P(4), ctypes.byref(mv), None) == tab.ERR_UNSUPPORTED
+    assert L.tabattn_mlp_fwd(0, 64, 128, 1.0, 0.0, P(0), P(1), P(2), P(3), P(4), ctypes.byref(mv), None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_mlp_fwd(100, 64, 128, 1.0, 0.0, P(0), P(1), P(2), P(3), P(0), ctypes.byref(mv), None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_mlp_workspace_bytes(100, 64, 128) > 100 * 128 * 4
+    assert L.tabattn_mlp_workspace_bytes(100, 60, 128) == 0
+    # Newton-Schulz: m <= n, multiples of 8, workspace checked
+    assert L.tabattn_newton_schulz(2, 64, 32, P(0), P(1), 5, P(2), 1 << 20, None) == tab.ERR_UNSUPPORTED
+    assert L.tabattn_newton_schulz(2, 60, 64, P(0), P(1), 5, P(2), 1 << 20, None) == tab.ERR_UNSUPPORTED
+    assert L.tabattn_newton_schulz(2, 64, 64, P(0), P(0), 5, P(2), 1 << 20, None) == tab.ERR_INVALID_ARG
+    assert L.tabattn_newton_schulz(2, 64, 64, P(0), P(1), 5, None, 0, None) == tab.ERR_WORKSPACE
+    assert L.tabattn_newton_schulz_workspace_bytes(2, 64, 64) >= (2 * 64 * 64 * 3) * 2
