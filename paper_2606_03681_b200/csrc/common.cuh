@@ -144,6 +144,28 @@ __host__ __device__ constexpr bool pair_is_poly(int k) {
   return ((k % 8) * POLY_OF_8) / 8 != (((k % 8) + 1) * POLY_OF_8) / 8;
 }
 
+// Timeline instrumentation (only with -DTABATTN_TRACE, `TABATTN_TRACE=1 python -m paper_2606_03681_b200.build`; the
+// shipped library has none of it): clock64() stamps of CTA 0's first 64 steps, event e of step n at trace[16 n + e].
+// A kernel file that traces says TABATTN_TRACE_DEFINE(setter) once at namespace scope (its own buffer pointer and
+// exported setter); paper_2606_03681_b200/trace_feature_bwd.py prints a trace; profiles/r02_attention.md has the
+// reading that found the LSU jam of the per-thread row stores.
+#ifdef TABATTN_TRACE
+#define TABATTN_TRACE_DEFINE(setter)                                                                      \
+  static __device__ long long* g_trace = nullptr;                                                         \
+  extern "C" __attribute__((visibility("default"))) void setter(long long* p) {                            \
+    cudaMemcpyToSymbol(g_trace, &p, sizeof(p));                                                            \
+  }
+// TR_INIT() once per kernel (reads the buffer pointer into a register: a stamp must not wait for a global load;
+// measured ~200 clk per stamp with the load, which distorted what it timed)
+#define TR_INIT() long long* const tr_buf_ = blockIdx.x == 0 ? g_trace : nullptr
+#define TR(ev, tile) \
+  do { if (tr_buf_ && (tile) < 64) tr_buf_[(tile) * 16 + (ev)] = clock64(); } while (0)
+#else
+#define TABATTN_TRACE_DEFINE(setter)
+#define TR_INIT() do { } while (0)
+#define TR(ev, tile) do { } while (0)
+#endif
+
 // 4 x 4 transpose of 16-byte chunks among the four lanes of a quad: on return lane i of the quad holds in a[k] the
 // chunk i that lane k of the quad passed in.  It turns "every lane stores its own 64-byte row in four instructions"
 // (32 different lines per instruction) into "a quad stores one row per instruction" (8 lines per instruction): the

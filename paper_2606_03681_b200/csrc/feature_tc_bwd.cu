@@ -27,20 +27,7 @@
 
 namespace tabattn {
 
-// Timeline instrumentation (only with -DTABATTN_TRACE, `TABATTN_TRACE=1 python -m paper_2606_03681_b200.build`; the
-// shipped library has none of it): clock64() stamps of CTA 0's first 64 tiles, event e of tile n at trace[16 n + e].
-// paper_2606_03681_b200/trace_feature_bwd.py prints them; profiles/r02_attention.md has the reading that found the
-// LSU jam of the per-thread row stores.
-#ifdef TABATTN_TRACE
-__device__ long long* g_trace = nullptr;
-extern "C" __attribute__((visibility("default"))) void tabattn_debug_set_trace(long long* p) {
-  cudaMemcpyToSymbol(g_trace, &p, sizeof(p));
-}
-#define TR(ev, tile) \
-  do { if (blockIdx.x == 0 && (tile) < 64 && g_trace) g_trace[(tile) * 16 + (ev)] = clock64(); } while (0)
-#else
-#define TR(ev, tile) do { } while (0)
-#endif
+TABATTN_TRACE_DEFINE(tabattn_debug_set_trace)
 
 namespace {
 
@@ -86,6 +73,7 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
                       const unsigned char* __restrict__ K, const unsigned char* __restrict__ V,
                       const unsigned char* __restrict__ dO, const float* __restrict__ LSE,
                       unsigned char* __restrict__ dQ, unsigned char* __restrict__ dK, unsigned char* __restrict__ dV) {
+  TR_INIT();
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE = Cfg::TILE, ROWB = Cfg::ROWB, STAGE = Cfg::STAGE, NSETS = Cfg::NSETS;
   extern __shared__ uint8_t smem_raw[];

@@ -41,6 +41,8 @@
 
 namespace tabattn {
 
+TABATTN_TRACE_DEFINE(tabattn_debug_set_trace_item_bwd)
+
 namespace {
 
 int item_bwd_padded_rows(const Shape& s);
@@ -129,6 +131,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
                    float* lse2_ws, float* D_ws, uint4* Drec_ws, __nv_bfloat16* __restrict__ out0,
                    __nv_bfloat16* __restrict__ out1, const uint32_t* __restrict__ col_list, int n_items_all,
                    int blocks_per_seq, int Rp) {
+  TR_INIT();
   using Cfg = BwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE_A = Cfg::TILE_A, TILE_B = Cfg::TILE_B, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -261,6 +264,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
         mbar_wait(b_b_full + 8 * st, ph);
+        if (lane == 0 && g == 0 && (t >> 1) < 32) TR(10, (int)(t >> 1) + 32 * MODE);   // chunk landed
         if (MODE == MODE_DQ) {
           // keys >= n must not reach dQ through dS K: zero the K rows beyond n (dS is forced to 0 there,
           // but 0 x NaN would still be NaN).  Ordered before the accumulation MMAs of this chunk through
@@ -269,6 +273,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           if (rem < kChunk) zero_tail_rows<ROWB, kChunk>(sB + st * Cfg::STAGE, rem, lane);
         }
         mbar_wait(b_s_empty + 8 * g, ((t >> 1) & 1) ^ 1);
+        if (lane == 0 && g == 0 && (t >> 1) < 32) TR(11, (int)(t >> 1) + 32 * MODE);   // set free
         tc_fence_after();
         const uint32_t set = tmem + g * Cfg::SET;
         const uint64_t b1 = dB + (st * Cfg::STAGE >> 4), b2 = b1 + (TILE_B >> 4);
@@ -282,6 +287,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           else mma_ss_e(set + Cfg::DP_OFF, dOnes, dRecB + (st * Cfg::DB_BYTES >> 4), idesc, 1u);
         }
         tc_commit_e(b_s_full + 8 * g);
+        if (lane == 0 && g == 0 && (t >> 1) < 32) TR(12, (int)(t >> 1) + 32 * MODE);   // S / dP issued
         if (j == it.chunks - 1) tc_commit_e(b_a_empty + 8 * ab);
         if (++st == ST) { st = 0; ph ^= 1; }
       }
@@ -307,6 +313,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
         mbar_wait(b_p_full + 8 * g, (t >> 1) & 1);
+        if (lane == 0 && first && g == 0 && (t >> 1) < 32) TR(13, (int)(t >> 1) + 32 * MODE);   // P / dS ready
         tc_fence_after();
         const uint32_t a = tmem + g * Cfg::SET + acol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -315,6 +322,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           mma_ts_e(acc, a + 8 * kk, b + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
         tc_commit_e(b_p_empty + 8 * g);
         tc_commit_e(b_b_empty + 8 * st);
+        if (lane == 0 && first && g == 0 && (t >> 1) < 32) TR(14, (int)(t >> 1) + 32 * MODE);   // accumulation issued
         if (j == it.chunks - 1) tc_commit_e(smem_u32(&bar_acc_full));
         if (++st == ST) st = 0;
       }
@@ -515,6 +523,9 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {
         const uint32_t u = (tbase + j) >> 1;  // this set's chunk counter
         mbar_wait(b_s_full, u & 1);
+        const int tbv = 5 * (g + 2 * c), tst = (int)u + 32 * MODE;   // (trace slots)
+        if (r == 0 && u < 32 && tbv < 10) TR(tbv + 0, tst);     // S / dP ready
+        if (r == 0 && u < 32 && tbv == 0) TR(15, tst);          // (calibration: cost of one stamp)
         tc_fence_after();
         uint32_t sr[32], dr[32];
         tmem_ld32(set + Cfg::S_OFF + 32 * c, sr);
@@ -529,6 +540,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         float c2d = c2;
         if constexpr (DH >= 64) c2d = mbar_arrive_then(b_s_empty, lane == 0, c2);
         else if (lane == 0) mbar_arrive(b_s_empty);
+        if (r == 0 && u < 32 && tbv < 10) TR(tbv + 1, tst);     // S / dP loaded, set released
         const uint64_t cc = f2pack(c2d, c2d);
         uint32_t pds[16], pp[16];
         if (MODE == MODE_DQ) {
@@ -581,13 +593,16 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
             pds[(k >> 1) + 1] = pack_bf16(d2, d3);
           }
         }
+        if (r == 0 && u < 32 && tbv < 10) TR(tbv + 2, tst);     // arithmetic done
         mbar_wait(b_p_empty, (u & 1) ^ 1);  // the MMAs that read this set's previous P/dS are done
+        if (r == 0 && u < 32 && tbv < 10) TR(tbv + 3, tst);     // P / dS columns free
         tmem_st16(set + Cfg::DS_OFF + 16 * c, pds);
         if (MODE == MODE_DKV) tmem_st16(set + Cfg::P_OFF + 16 * c, pp);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(b_p_full);
+        if (r == 0 && u < 32 && tbv < 10) TR(tbv + 4, tst);     // P / dS stored
         if (pend) {
           epilogue(p_cell, p_row, p_n, p_par);
           pend = false;

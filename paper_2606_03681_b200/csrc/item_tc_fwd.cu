@@ -22,6 +22,8 @@
 
 namespace tabattn {
 
+TABATTN_TRACE_DEFINE(tabattn_debug_set_trace_item_fwd)
+
 namespace {
 
 using namespace tc;
@@ -51,6 +53,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                    const __grid_constant__ CUtensorMap mapV, Shape s, __nv_bfloat16* __restrict__ O,
                    float* __restrict__ LSE, const uint32_t* __restrict__ col_list, int n_items_all,
                    int blocks_per_seq, int q_row0, int q_row1) {
+  TR_INIT();
   using Cfg = FwdCfg<DH>;
   constexpr int ST = Cfg::ST, TILE = Cfg::TILE, ROWB = Cfg::ROWB;
   extern __shared__ uint8_t smem_raw[];
@@ -268,6 +271,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       float m = -INFINITY, l = 0.f;
       for (int j = 0; j < tiles; ++j, ++g) {
         mbar_wait(b_s_full, g & 1);
+        if (r == 0) TR(0 + 7 * t, g);                      // S ready
         tc_fence_after();
         uint32_t sr[128];
         tmem_ld32(tS, sr);
@@ -277,6 +281,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         tmem_wait_ld();
         tc_fence_before();
         mbar_arrive(b_s_empty);
+        if (r == 0) TR(1 + 7 * t, g);                      // S loaded, buffer released
         float* sf = reinterpret_cast<float*>(sr);
         const int rem = it.n - j * kTileRows;
         if (rem < kTileRows) {
@@ -315,6 +320,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
         // P = 2^(S*c2 - m) on packed pairs; Cfg::POLY_OF_8 of every 8 pairs take the FMA-pipe polynomial, the
         // rest the MUFU, so that the two pipes finish together
+        if (r == 0) TR(2 + 7 * t, g);                      // maximum done
         const uint64_t cc = f2pack(c2, c2), nm = f2pack(-m, -m);
         uint64_t la = 0, lb = 0;  // two packed partial row sums (+0.f, +0.f)
         uint32_t p[64];
@@ -331,15 +337,19 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           f2unpack(add2(la, lb), s0, s1);
           l += s0 + s1;
         }
+        if (r == 0) TR(3 + 7 * t, g);                      // exponentials done
         if (g > 0) mbar_wait(b_pv_done, (g - 1) & 1);  // previous PV has finished reading the P buffer
+        if (r == 0) TR(4 + 7 * t, g);                      // P buffer free
         tmem_st32(tP, p);
         tmem_st32(tP + 32, p + 32);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(b_p_full);
+        if (r == 0) TR(5 + 7 * t, g);                      // P stored
       }
       // ---- epilogue: O = acc / l, LSE = ln(sum exp) ---------------------------------------------
       mbar_wait(b_pv_done, (g - 1) & 1);
+      if (threadIdx.x == 0) TR(14, g - 1);                 // last PV of the item done
       tc_fence_after();
       uint32_t o[DH];
       tmem_ld_cols<DH>(tO, o);
@@ -379,6 +389,7 @@ item_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
         if (LSE) *lse = (m + log2f(l)) * kLn2;
       }
+      if (threadIdx.x == 0) TR(15, g - 1);                 // O and LSE stored
       if (MASKED && wz < n_zero) zero_one();
     }
     while (MASKED && wz < n_zero) zero_one();   // (what is left of the invalid columns)

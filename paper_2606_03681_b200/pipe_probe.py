@@ -1,0 +1,26 @@
+"""Build and run probes/pipe_probe.cu (developer tool; needs a B200): issue cost of the instructions of the softmax
+loops and of the forward kernel's row step on one SM sub-partition.
+
+    python -m paper_2606_03681_b200.pipe_probe
+
+The binary goes to a temporary directory; nothing of it is part of libtabattn.so.
+"""
+import os
+import subprocess
+import sys
+import tempfile
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def main():
+    src = os.path.join(HERE, "probes", "pipe_probe.cu")
+    with tempfile.TemporaryDirectory() as tmp:
+        exe = os.path.join(tmp, "pipe_probe")
+        subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                        "-o", exe, src], check=True)
+        return subprocess.run([exe]).returncode
+
+
+if __name__ == "__main__":
+    sys.exit(main())
