@@ -313,7 +313,6 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
       for (int j = 0; j < it.chunks; ++j, ++t) {
         const uint32_t g = t & 1;
         mbar_wait(b_p_full + 8 * g, (t >> 1) & 1);
-        if (lane == 0 && first && g == 0 && (t >> 1) < 32) TR(13, (int)(t >> 1) + 32 * MODE);   // P / dS ready
         tc_fence_after();
         const uint32_t a = tmem + g * Cfg::SET + acol;
         const uint64_t b = dB + (st * Cfg::STAGE >> 4);
@@ -322,7 +321,6 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
           mma_ts_e(acc, a + 8 * kk, b + kk * ROWB, idesc, (j > 0 || kk > 0) ? 1u : 0u);
         tc_commit_e(b_p_empty + 8 * g);
         tc_commit_e(b_b_empty + 8 * st);
-        if (lane == 0 && first && g == 0 && (t >> 1) < 32) TR(14, (int)(t >> 1) + 32 * MODE);   // accumulation issued
         if (j == it.chunks - 1) tc_commit_e(smem_u32(&bar_acc_full));
         if (++st == ST) st = 0;
       }
@@ -508,6 +506,8 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         }
         continue;
       }
+      const int tfirst = (int)((tbase + ((g ^ tbase) & 1)) >> 1) + 32 * MODE;   // (trace slot of the item's first chunk)
+      if (threadIdx.x == 0 && tfirst - 32 * MODE < 32) TR(13, tfirst);   // item decoded
       // per-row constants of the dQ pass, from the stats warp (rows >= R: nlse2 = -inf -> P = 0)
       float nlse2 = -INFINITY, Drow = 0.f;
       if (MODE == MODE_DQ) {
@@ -518,6 +518,7 @@ item_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapA1, const __grid_const
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&bar_d_empty[db]));
       }
+      if (threadIdx.x == 0 && tfirst - 32 * MODE < 32) TR(14, tfirst);   // row statistics read
       const uint64_t nl = f2pack(nlse2, nlse2), dd = f2pack(Drow, Drow);
       const int chunks = it.chunks;
       for (int j = (g ^ tbase) & 1; j < chunks; j += 2) {

@@ -8,7 +8,8 @@ Prints, for the first 32 chunk steps of each TMEM set of CTA 0 in the dQ pass an
 clock64() stamps (relative to the pass's first one) of the events named in csrc/item_tc_bwd.cu (TR(...)): S / dP
 ready, loaded (set released), arithmetic done, P / dS columns free, P / dS stored -- for the warpgroups (set 0, columns
 0-31) and (set 1, columns 0-31) -- then, for set 0's chunks, the S / dP issue warp (chunk landed, set free, issued)
-and the first accumulation warp (P / dS ready, issued), and the step-to-step difference of the first column.
+the two stamps of warpgroup (0, 0) at the start of an item (item decoded, row statistics read; on the item's first
+chunk only), a second stamp right after the first (the cost of a stamp), and the step-to-step difference of the first column.
 """
 import ctypes
 import sys
@@ -19,7 +20,7 @@ import paper_2606_03681_b200 as tab
 from workloads import get_config, draw_structure, make_call_inputs
 
 EV = ["ready", "loaded", "math", "free", "stored"]
-NAMES = [e + w for w in ("00", "10") for e in EV] + ["landed", "setFree", "sIssued", "pReady", "accIss", "calib"]
+NAMES = [e + w for w in ("00", "10") for e in EV] + ["landed", "setFree", "sIssued", "decoded", "stats", "calib"]
 
 
 def main():
