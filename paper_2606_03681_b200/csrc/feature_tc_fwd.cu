@@ -110,14 +110,18 @@ __global__ void __launch_bounds__(256) feature_prep_kernel(Shape s, FeatTab* __r
 // scores there).  Before the first P store the thread drains the accumulator of the set's PREVIOUS tile
 // (`drain`): that tile's P V MMA finished long ago (the S MMA of this tile was issued behind it), so its
 // round trip is never waited for.
+// `nlive`: chunks of the window that hold live keys, ceil(Cv / 32).  A W = 128 window of a table with Cv <= 96 has a
+// whole chunk of masked keys, whose P is exactly zero: it is neither read nor exponentiated (feature_heavy: 65 % of
+// the tiles are one-row Cp = 128 tiles and 8 of 9 of those have Cv <= 96).
 template <int W, int DH>
-__device__ __forceinline__ void softmax_window(uint32_t tSwin, uint32_t tProw, int pgrp0, float c2, float& m_out,
-                                               float& l_out, bool drain, uint32_t tO, uint32_t (&o)[DH]) {
+__device__ __forceinline__ void softmax_window(uint32_t tSwin, uint32_t tProw, int pgrp0, int nlive, float c2,
+                                               float& m_out, float& l_out, bool drain, uint32_t tO, uint32_t (&o)[DH]) {
   constexpr int NCH = W / 32;
   uint32_t sr[32];
   float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
   for (int c = 0; c < NCH; ++c) {
+    if (NCH > 2 && c >= nlive) continue;
     tmem_ld32(tSwin + 32 * c, sr);
     tmem_wait_ld();
     const float* sf = reinterpret_cast<const float*>(sr);
@@ -138,6 +142,13 @@ __device__ __forceinline__ void softmax_window(uint32_t tSwin, uint32_t tProw, i
   }
 #pragma unroll
   for (int c = 0; c < NCH; ++c) {
+    if (NCH > 2 && c >= nlive) {
+      uint32_t z[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) z[k] = 0u;
+      tmem_st16(tProw + 16 * (pgrp0 + c), z);
+      continue;
+    }
     if (NCH > 1) {
       tmem_ld32(tSwin + 32 * c, sr);
       tmem_wait_ld();
@@ -447,9 +458,10 @@ feature_fwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       // the S MMA of this tile was issued behind the previous tile's P V MMA: the accumulator is ready
       tc_fence_after();
       float m, l;
-      if (x.lgCp <= 5) softmax_window<32, DH>(tS + colbase, tS, colbase >> 5, c2, m, l, pd_on, tO, o);
-      else if (x.lgCp == 6) softmax_window<64, DH>(tS + colbase, tS, colbase >> 5, c2, m, l, pd_on, tO, o);
-      else softmax_window<128, DH>(tS + colbase, tS, colbase >> 5, c2, m, l, pd_on, tO, o);
+      const int nlive = (x.Cv + 31) >> 5;
+      if (x.lgCp <= 5) softmax_window<32, DH>(tS + colbase, tS, colbase >> 5, nlive, c2, m, l, pd_on, tO, o);
+      else if (x.lgCp == 6) softmax_window<64, DH>(tS + colbase, tS, colbase >> 5, nlive, c2, m, l, pd_on, tO, o);
+      else softmax_window<128, DH>(tS + colbase, tS, colbase >> 5, nlive, c2, m, l, pd_on, tO, o);
       __syncwarp();
       if (lane == 0) mbar_arrive(b_p_full);
       if (pd_on) store_prev();
