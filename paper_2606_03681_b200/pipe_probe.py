@@ -13,13 +13,18 @@ import tempfile
 HERE = os.path.dirname(os.path.abspath(__file__))
 
 
-def main():
+def compile_probe(out_dir):
+    """nvcc probes/pipe_probe.cu for sm_100a into ``out_dir``; returns the path of the binary."""
     src = os.path.join(HERE, "probes", "pipe_probe.cu")
+    exe = os.path.join(out_dir, "pipe_probe")
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                    "-o", exe, src], check=True)
+    return exe
+
+
+def main():
     with tempfile.TemporaryDirectory() as tmp:
-        exe = os.path.join(tmp, "pipe_probe")
-        subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-                        "-o", exe, src], check=True)
-        return subprocess.run([exe]).returncode
+        return subprocess.run([compile_probe(tmp)]).returncode
 
 
 if __name__ == "__main__":
