@@ -98,6 +98,23 @@ TABATTN_API tabattn_status tabattn_feature_bwd(const tabattn_shape* shape, const
 TABATTN_API tabattn_status tabattn_item_fwd(const tabattn_shape* shape, const void* Q, const void* K, const void* V,
                                 void* O, float* LSE, void* ws, size_t ws_bytes, tabattn_stream stream);
 
+/* Item attention forward WITHOUT any allocation: the same computation, kernels and results as tabattn_item_fwd
+ * (PAPER.md item-axis attention; same argument meaning, layouts and errors), for callers
+ * that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it) and so have no
+ * workspace to pass.  The scratch of a masked call (the a0 column list, 4 * (B*C + 4) bytes) lives in a
+ * `static __device__` array inside the library, sized for B*C <= TABATTN_NOALLOC_MAX_BC column pairs (256 KiB + 256 B
+ * that every GPU loading the library holds until the process exits).  The call itself allocates nothing: no
+ * cudaMalloc / cudaFree / allocating library routine; the array's device address is looked up once per device
+ * (cudaGetSymbolAddress) on that device's first masked call.
+ *   - shape->col_valid != NULL and B*C > TABATTN_NOALLOC_MAX_BC  =>  TABATTN_ERR_WORKSPACE (the built-in scratch is
+ *     too small; nothing is launched).  Unmasked calls use no scratch and have no such limit.
+ *   - Every call on a device shares the one array; it keeps the previous call's contents, and each call rewrites all
+ *     of it that it reads (nothing has to start at zero).  Calls that overlap on the GPU (different streams, or
+ *     several host threads on different streams) RACE on it: serialise them (one stream, or events). */
+#define TABATTN_NOALLOC_MAX_BC 65536
+TABATTN_API tabattn_status tabattn_item_fwd_noalloc(const tabattn_shape* shape, const void* Q, const void* K,
+                                                    const void* V, void* O, float* LSE, tabattn_stream stream);
+
 /* Item attention backward: a dQ pass (it also computes D = rowsum(dO o O) and -LSE*log2(e) per query
  * row and leaves them in the workspace) and a separate dK/dV pass that reads them; two kernel
  * launches, deterministic, no atomics.  ws: tabattn_workspace_bytes(shape, TABATTN_OP_ITEM_BWD)

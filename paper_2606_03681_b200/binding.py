@@ -22,6 +22,7 @@ OP_FEATURE_FWD, OP_FEATURE_BWD, OP_ITEM_FWD, OP_ITEM_BWD = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, 1, 2, 3, 4
 
 EXPORTS = ("tabattn_feature_fwd", "tabattn_feature_bwd", "tabattn_item_fwd", "tabattn_item_bwd",
+           "tabattn_item_fwd_noalloc",
            "tabattn_feature_fwd_infer", "tabattn_item_fwd_infer", "tabattn_workspace_bytes",
            "tabattn_attn_block_fwd", "tabattn_attn_block_bwd", "tabattn_attn_block_workspace_bytes",
            "tabattn_mlp_fwd", "tabattn_mlp_bwd", "tabattn_mlp_workspace_bytes",
@@ -72,8 +73,9 @@ def lib():
         i32 = ctypes.c_int32
         L.tabattn_feature_fwd_infer.argtypes = [shp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
         L.tabattn_item_fwd_infer.argtypes = [shp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
+        L.tabattn_item_fwd_noalloc.argtypes = [shp, vp, vp, vp, vp, vp, vp]
         for f in (L.tabattn_feature_fwd, L.tabattn_item_fwd, L.tabattn_feature_bwd, L.tabattn_item_bwd,
-                  L.tabattn_feature_fwd_infer, L.tabattn_item_fwd_infer):
+                  L.tabattn_feature_fwd_infer, L.tabattn_item_fwd_infer, L.tabattn_item_fwd_noalloc):
             f.restype = ctypes.c_int
         f32, i64 = ctypes.c_float, ctypes.c_int64
         asv, msv = ctypes.POINTER(TabattnAttnSaved), ctypes.POINTER(TabattnMlpSaved)
@@ -247,6 +249,27 @@ def tabattn_item_fwd(Q, K, V, n_train, col_valid=None, softmax_scale=0.0, n_trai
         st = lib().tabattn_item_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
                                     _ptr(ws), nws, _stream(stream, Q.device))
     _raise(st, "tabattn_item_fwd")
+    return O, LSE
+
+
+NOALLOC_MAX_BC = 65536   # TABATTN_NOALLOC_MAX_BC
+
+
+def tabattn_item_fwd_noalloc(Q, K, V, n_train, col_valid=None, softmax_scale=0.0, n_train_host=None, O=None,
+                             LSE=None, stream=None):
+    """Item-axis attention forward with the scratch inside the library (tabattn.h: tabattn_item_fwd_noalloc): the
+    C call allocates nothing.  Pass preallocated ``O`` / ``LSE`` to keep the whole call allocation-free; masked calls
+    need B*C <= NOALLOC_MAX_BC; calls that overlap on the GPU race on the shared scratch."""
+    _check_inputs(Q, K, V, O)
+    B, R, C, H, dh = Q.shape
+    _check_aux(Q, n_train, col_valid, LSE, (B, C, H, R))
+    shape, keep = make_shape(Q, n_train, col_valid, n_train_host, softmax_scale)
+    O = torch.empty_like(Q) if O is None else O
+    LSE = torch.empty((B, C, H, R), dtype=torch.float32, device=Q.device) if LSE is None else LSE
+    with _on(Q.device):
+        st = lib().tabattn_item_fwd_noalloc(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(LSE),
+                                            _stream(stream, Q.device))
+    _raise(st, "tabattn_item_fwd_noalloc")
     return O, LSE
 
 

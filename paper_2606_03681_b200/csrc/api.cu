@@ -167,6 +167,25 @@ tabattn_status tabattn_item_fwd(const tabattn_shape* sh, const void* Q, const vo
   return from_cuda(tabattn::launch_item_fwd(s, Q, K, V, O, LSE, 0, s.R, ws, (cudaStream_t)stream));
 }
 
+tabattn_status tabattn_item_fwd_noalloc(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
+                                        float* LSE, tabattn_stream stream) {
+  Shape s;
+  tabattn_status st = check_shape(sh, true, &s);
+  if (st != TABATTN_OK) return st;
+  if (!all_ok(Q, K, V, (const void*)O, (const void*)LSE)) return TABATTN_ERR_INVALID_ARG;
+  {
+    const void* const outs[] = {O, LSE};
+    const void* const ins[] = {Q, K, V};
+    if (aliased(outs, ins)) return TABATTN_ERR_INVALID_ARG;
+  }
+  // the column list of a masked call must fit the library's own device array (TABATTN_NOALLOC_MAX_BC pairs)
+  if (s.col_valid && ((long long)s.B * s.C > TABATTN_NOALLOC_MAX_BC ||
+                      tabattn::item_fwd_workspace_bytes(s) > tabattn::item_fwd_noalloc_capacity()))
+    return TABATTN_ERR_WORKSPACE;
+  if ((st = check_device()) != TABATTN_OK) return st;
+  return from_cuda(tabattn::launch_item_fwd_noalloc(s, Q, K, V, O, LSE, (cudaStream_t)stream));
+}
+
 tabattn_status tabattn_feature_fwd_infer(const tabattn_shape* sh, const void* Q, const void* K, const void* V, void* O,
                                          int32_t row0, int32_t row1, void* ws, size_t ws_bytes,
                                          tabattn_stream stream) {

@@ -16,7 +16,9 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <atomic>
 
+#include "../../include/tabattn.h"
 #include "item_tc_common.cuh"
 #include "kernels.h"
 
@@ -489,6 +491,51 @@ cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const 
     case 64: return launch_fwd<64>(s, Q, K, V, O, LSE, q_row0, q_row1, ws, stream);
     default: return cudaErrorInvalidValue;
   }
+}
+
+// ---- tabattn_item_fwd_noalloc: the same forward with its scratch inside the library -----------------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the a0
+// column list of a masked call lives in a file-scope device array instead of a caller workspace.  Every GPU that
+// loads the library holds the array (256 KiB + 256 B) until the process exits.  Nothing in it has to start at zero:
+// item_prep_kernel rewrites the count and every list entry the main kernel reads, on the call's stream, before the
+// main kernel runs.  All calls share the array, so two calls that overlap on the GPU (different streams) race.
+constexpr size_t kNoAllocScratchBytes = ((size_t)TABATTN_NOALLOC_MAX_BC + 4) * sizeof(uint32_t) + 240;
+static __device__ __align__(256) unsigned char g_item_fwd_scratch[kNoAllocScratchBytes];
+
+size_t item_fwd_noalloc_capacity() { return kNoAllocScratchBytes; }
+
+namespace {
+// In host code `g_item_fwd_scratch` is only the symbol's host-side stand-in: the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+struct ScratchAddr {
+  std::atomic<void*> ptr[kMaxDevices];
+  ScratchAddr() { for (auto& p : ptr) p.store(nullptr, std::memory_order_relaxed); }
+  cudaError_t get(int ordinal, void** out) {
+    void* p = ptr[ordinal].load(std::memory_order_acquire);
+    if (!p) {
+      const cudaError_t e = cudaGetSymbolAddress(&p, g_item_fwd_scratch);   // (the calling thread's current device)
+      if (e != cudaSuccess) return e;
+      if (!p) return cudaErrorInvalidSymbol;
+      ptr[ordinal].store(p, std::memory_order_release);   // (a lost race stores the same address twice)
+    }
+    *out = p;
+    return cudaSuccess;
+  }
+};
+ScratchAddr g_scratch_addr;
+}  // namespace
+
+cudaError_t launch_item_fwd_noalloc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
+                                    cudaStream_t stream) {
+  void* scratch = nullptr;
+  if (s.col_valid) {   // (an unmasked call has no scratch)
+    if (item_fwd_workspace_bytes(s) > kNoAllocScratchBytes) return cudaErrorInvalidValue;   // (the ABI checks first)
+    const DeviceInfo* di = current_device();
+    if (!di) return cudaErrorInvalidDevice;
+    const cudaError_t e = g_scratch_addr.get(di->ordinal, &scratch);
+    if (e != cudaSuccess) return e;
+  }
+  return launch_item_fwd(s, Q, K, V, O, LSE, 0, s.R, scratch, stream);
 }
 
 }  // namespace tabattn

@@ -30,6 +30,11 @@ size_t feature_workspace_bytes(const Shape& s);   // masked calls: per-table geo
 cudaError_t launch_item_fwd(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
                             int q_row0, int q_row1, void* ws, cudaStream_t stream);
 size_t item_fwd_workspace_bytes(const Shape& s);
+// tabattn_item_fwd_noalloc: the forward over all rows with the column list in the library's own device array
+// (item_tc_fwd.cu); a masked call needs item_fwd_workspace_bytes(s) <= item_fwd_noalloc_capacity()
+cudaError_t launch_item_fwd_noalloc(const Shape& s, const void* Q, const void* K, const void* V, void* O, float* LSE,
+                                    cudaStream_t stream);
+size_t item_fwd_noalloc_capacity();
 cudaError_t launch_item_bwd(const Shape& s, const void* Q, const void* K, const void* V, const void* O,
                             const void* dO, const float* LSE, void* dQ, void* dK, void* dV, float* ws,
                             cudaStream_t stream);
