@@ -40,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     compile_flags = [f for f in NVCC_FLAGS if f not in ("-shared",)]
-    if os.environ.get("TABATTN_TRACE"):      # developer build with the timeline stamps of feature_tc_bwd.cu
+    if os.environ.get("TABATTN_TRACE"):      # developer build with the timeline stamps (TR(...) in the kernels)
         compile_flags.append("-DTABATTN_TRACE")
     for src in sources():
         obj = os.path.join(objdir, os.path.basename(src) + ".o")

@@ -352,6 +352,9 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
       const bool first_tile = g == 0 && k == 0;
 
       auto body = [&](auto WC) {
+        // W = 96: a Cp = 128 window whose last 32 columns are masked keys only (Cv <= 96; P = dS = 0 there exactly):
+        // three chunks are computed and the fourth is stored as zeros.  Its own instantiation, so that the loops keep
+        // compile-time bounds (a run-time chunk count in the W = 128 body spilled 104 bytes and lost 5-8 %).
         constexpr int W = decltype(WC)::value, NCH = W / 32;
         constexpr int NREG = NCH > 2 ? 2 : NCH;            // chunks of packed P kept in registers
         uint32_t pp[16 * NREG];
@@ -496,9 +499,16 @@ feature_bwd_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
           }
           store_chunk(c, pk, ds);
         }
+        if constexpr (W == 96) {
+          uint32_t z[16];
+#pragma unroll
+          for (int q = 0; q < 16; ++q) z[q] = 0u;
+          store_chunk(3, z, z);
+        }
       };
       if (x.lgCp <= 5) body(std::integral_constant<int, 32>{});
       else if (x.lgCp == 6) body(std::integral_constant<int, 64>{});
+      else if (x.Cv <= 96) body(std::integral_constant<int, 96>{});
       else body(std::integral_constant<int, 128>{});
       tc_fence_before();
       fence_proxy_async_smem();
