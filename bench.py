@@ -459,7 +459,28 @@ def time_next_rows(torch, tab, dev, peaks, iters=20):
     fl = nb * 5 * 6 * m ** 3
     out["newton_schulz"] = {"nb": nb, "m": m, "n": m, "steps": 5, "ms": tns, "TFLOP/s": fl / tns / 1e9,
                             "launches": 16, "note": "30 matrices of 256x256 (3.9 MB): L2-resident and launch-bound"}
+    out["tiny_layer"] = time_tiny_layer(torch, tab, dev)
     return out
+
+
+def time_tiny_layer(torch, tab, dev, iters=1000):
+    """configs[0] (Tiny, 2 x 64 x 6 cells) is launch-bound: one layer through the four ctypes calls against the same
+    four calls captured in a CUDA graph (tab.LayerGraph) and replayed.  Not a throughput claim: host overhead."""
+    from workloads import get_config, draw_structure, make_call_inputs
+    cfg = get_config("tiny")
+    nt_h, cv_h = draw_structure(cfg)
+    nt = torch.from_numpy(nt_h).to(dev)
+    cv = torch.from_numpy(cv_h).to(dev) if cv_h is not None else None
+    feat = make_call_inputs(cfg, "feature", 0, device=dev)
+    item = make_call_inputs(cfg, "item", 0, device=dev)
+    buf = tab.LayerBuffers(cfg.B, cfg.R, cfg.C, cfg.H, cfg.dh, device=dev)
+    stream = torch.cuda.current_stream()
+    direct = _timeit(torch, stream, lambda: tab.layer_fwd_bwd(feat, item, nt, cv, buf, n_train_host=nt_h), iters, 20)
+    graph = tab.LayerGraph(feat, item, nt, cv, buf, n_train_host=nt_h)
+    replay = _timeit(torch, stream, graph.replay, iters, 20)
+    return {"workload": "tiny", "direct_us_per_layer": direct * 1e3, "graph_us_per_layer": replay * 1e3,
+            "kernels_per_replay": graph.kernels_per_replay,
+            "note": "launch-bound: the direct figure is the host cost of four ctypes calls, the graph figure one replay"}
 
 
 def static_traffic(cfg_name, call):

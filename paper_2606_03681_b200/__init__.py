@@ -13,12 +13,12 @@ from .binding import (TabattnError, TabattnShape, EXPORTS, LIB_PATH, lib, make_s
                       OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA)
 from .binding import (tabattn_attn_block_fwd, tabattn_attn_block_bwd, tabattn_mlp_fwd, tabattn_mlp_bwd,
                       tabattn_newton_schulz, AttnSaved, MlpSaved)
-from .layer import LayerBuffers, layer_fwd_bwd, layer_fwd_bwd_host
+from .layer import LayerBuffers, LayerGraph, layer_fwd_bwd, layer_fwd_bwd_host
 
 __all__ = [
     "TabattnError", "TabattnShape", "EXPORTS", "LIB_PATH", "lib", "make_shape", "status_string", "version", "launch_count",
     "workspace_bytes", "tabattn_feature_fwd", "tabattn_feature_bwd", "tabattn_item_fwd", "tabattn_item_bwd",
     "tabattn_feature_fwd_infer", "tabattn_item_fwd_infer", "tabattn_item_fwd_noalloc", "NOALLOC_MAX_BC",
     "tabattn_attn_block_fwd", "tabattn_attn_block_bwd",
-    "tabattn_mlp_fwd", "tabattn_mlp_bwd", "tabattn_newton_schulz", "AttnSaved", "MlpSaved", "LayerBuffers", "layer_fwd_bwd", "layer_fwd_bwd_host",
+    "tabattn_mlp_fwd", "tabattn_mlp_bwd", "tabattn_newton_schulz", "AttnSaved", "MlpSaved", "LayerBuffers", "LayerGraph", "layer_fwd_bwd", "layer_fwd_bwd_host",
 ]
