@@ -457,7 +457,17 @@ def time_next_rows(torch, tab, dev, peaks, iters=20):
     wsn = torch.empty(int(tab.lib().tabattn_newton_schulz_workspace_bytes(nb, m, m)), dtype=torch.uint8, device=dev)
     tns = _timeit(torch, stream, lambda: tab.tabattn_newton_schulz(G, 5, X=X, ws=wsn), iters)
     fl = nb * 5 * 6 * m ** 3
+    # the same call captured in a CUDA graph (it allocates nothing): what the 16 launches cost without the host
+    side = torch.cuda.Stream()
+    side.wait_stream(stream)
+    with torch.cuda.stream(side):
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr, stream=side):
+            tab.tabattn_newton_schulz(G, 5, X=X, ws=wsn)
+    stream.wait_stream(side)
+    tng = _timeit(torch, stream, gr.replay, iters)
     out["newton_schulz"] = {"nb": nb, "m": m, "n": m, "steps": 5, "ms": tns, "TFLOP/s": fl / tns / 1e9,
+                            "graph_ms": tng, "graph_TFLOP/s": fl / tng / 1e9,
                             "launches": 16, "note": "30 matrices of 256x256 (3.9 MB): L2-resident and launch-bound"}
     out["tiny_layer"] = time_tiny_layer(torch, tab, dev)
     return out
