@@ -1,11 +1,15 @@
-// tcgen05 GEMM core (gemm_tc.cuh): one 128 x BN output tile per CTA, a 2-3 stage TMA ring over 64-wide k-blocks,
-// fp32 accumulator in TMEM, fused epilogue, TMA store.  Warp 0 = TMA producer (one lane), warp 1 = MMA issuer
-// (owns the TMEM allocation), warps 2-9 = epilogue (one thread per accumulator row and column half).  Two CTAs fit an SM,
-// so one tile's epilogue overlaps the other's main loop; these contractions have K = 192..768 only and
-// are bound by HBM and the epilogue, not by the tensor pipe.
+// tcgen05 GEMM core (gemm_tc.cuh): 128 x BN output tiles, a 2-3 stage TMA ring over 64-wide k-blocks, fp32 accumulators
+// in TMEM, fused epilogue, TMA store.  Warp 0 = TMA producer (one lane), warp 1 = MMA issuer (owns the TMEM
+// allocation), warps 2-9 = epilogue (one thread per accumulator row and column half).  A CTA is persistent over the
+// row tiles of its column tile and alternates TWO accumulators, so that tile i's epilogue (TMEM -> registers -> staging
+// tile -> TMA store) runs under tile i+1's loads and MMAs; two such CTAs fit an SM (96 KB of shared memory and 256
+// TMEM columns each at BN = 128).  These contractions have K = 192..768 only: a tile is 4-12 k-blocks of work and the
+// kernels are bound by HBM and the epilogue, not by the tensor pipe (profiles/r02_blocks.md).
 #include "gemm_tc.cuh"
 
 #include <cudaTypedefs.h>
+
+#include <algorithm>
 
 #include "common.cuh"
 #include "device.h"
@@ -74,19 +78,17 @@ __device__ __forceinline__ float gelu_grad_f(float x) {
 
 template <int BN>
 struct Cfg {
-  static constexpr int ST = BN == 64 ? 3 : 2;   // two CTAs per SM: one tile's epilogue overlaps the other's main loop
+  static constexpr int ST = BN == 64 ? 3 : 2;
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE = A_BYTES + B_BYTES;
   static constexpr int STAGING = (BN / 64) * (BM * 128);
-  // the epilogue's staging tile: its own buffer when an auxiliary tile is prefetched into it, else it aliases the
-  // (by then idle) A stages, which lets a third CTA fit an SM
+  // the epilogue's staging tile is a buffer of its own (an auxiliary tile is prefetched into it when there is one):
+  // the ring keeps loading the next tile while the epilogue of the current one writes it
   static constexpr int SMEM_AUX = ST * STAGE + STAGING + 1024;
-  static constexpr int SMEM_MAIN = ST * STAGE + 1024;
-  static_assert(STAGING <= ST * A_BYTES, "staging aliases the A stages");
 };
 
 template <int BN, int A_MN, int B_MN>
-__global__ void __launch_bounds__(kThreads, 3)
+__global__ void __launch_bounds__(kThreads, 2)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA2,
                const __grid_constant__ CUtensorMap mapA3, const __grid_constant__ CUtensorMap mapB,
                const __grid_constant__ CUtensorMap mapAux, const __grid_constant__ CUtensorMap mapC0,
@@ -97,24 +99,31 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = sbase, sB = sA + ST * A_BYTES;
-  const uint32_t sOut = p.aux_mode != AUX_NONE ? sB + ST * C::B_BYTES : sA;
-  __shared__ uint64_t bar_full[ST], bar_empty[ST], bar_acc, bar_aux;
+  const uint32_t sOut = sB + ST * C::B_BYTES;   // the epilogue's staging tile (the auxiliary tile lands in it first)
+  __shared__ uint64_t bar_full[ST], bar_empty[ST], bar_acc[2], bar_aux, bar_acc_free[2], bar_out_free;
   __shared__ uint32_t tmem_slot;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
-  const int n0 = blockIdx.x * BN, m0 = blockIdx.y * BM;
+  // A CTA walks the row tiles my = blockIdx.y, blockIdx.y + gridDim.y, ... of its column tile (the host sizes
+  // gridDim.y so that all CTAs are resident at once): TMEM allocation, barrier set-up and the CTA launch are paid once
+  // per CTA instead of once per 128 x BN tile -- with K = 256..768 a tile is only 4-12 k-blocks of work.
+  const int n0 = blockIdx.x * BN, tiles_m = (p.M + BM - 1) / BM;
   const bool splitk = p.partial != nullptr;   // fp32 partial tiles instead of the bf16 output
   const int bz = splitk ? 0 : blockIdx.z, slab = splitk ? blockIdx.z : 0;
   const int kb0 = slab * p.kb_per_slab, kb1 = min(p.kb_total, kb0 + p.kb_per_slab);
 
-  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), BN);
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), 2 * BN);   // two accumulators: tile i's epilogue under tile i+1's MMAs
   if (threadIdx.x == 0) {
     for (int i = 0; i < ST; ++i) {
       mbar_init(smem_u32(&bar_full[i]), 1);
       mbar_init(smem_u32(&bar_empty[i]), 1);
     }
-    mbar_init(smem_u32(&bar_acc), 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&bar_acc[i]), 1);
+      mbar_init(smem_u32(&bar_acc_free[i]), kEpiWarps);   // the epilogue warps have read the accumulator
+    }
     mbar_init(smem_u32(&bar_aux), 1);
+    mbar_init(smem_u32(&bar_out_free), 1);           // the tile's store has read the staging tile
     fence_barrier_init();
   }
   tc_fence_before();
@@ -127,13 +136,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       tma_prefetch_desc(&mapA);
       tma_prefetch_desc(&mapB);
       const int ba = p.a_batched ? bz : 0, bb = p.b_batched ? bz : 0;
-      if (p.aux_mode != AUX_NONE) {
-        // the tile of the auxiliary operand lands in the staging tile the epilogue later overwrites in place
-        mbar_arrive_expect_tx(smem_u32(&bar_aux), C::STAGING);
-#pragma unroll
-        for (int h = 0; h < BN / 64; ++h) tma_load_3d(sOut + h * (BM * 128), &mapAux, smem_u32(&bar_aux), n0 + 64 * h, m0, bz);
-      }
-      uint32_t t = 0;
+      uint32_t t = 0, it = 0;
+      for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
+      const int m0 = my * BM;
+      // (the A / B loads of a tile run ahead under the previous tile's epilogue; the auxiliary load, below, waits for
+      // the staging tile)
       for (int kb = kb0; kb < kb1; ++kb, ++t) {
         const uint32_t st = t % ST, full = smem_u32(&bar_full[st]);
         mbar_wait<true>(smem_u32(&bar_empty[st]), ((t / ST) & 1) ^ 1);
@@ -155,6 +162,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           tma_load_3d(b, &mapB, full, kb * BK, n0, bb);
         }
       }
+      if (p.aux_mode != AUX_NONE) {
+        // the tile of the auxiliary operand lands in the staging tile the epilogue later overwrites in place
+        if (it > 0) mbar_wait<true>(smem_u32(&bar_out_free), (it - 1) & 1);
+        mbar_arrive_expect_tx(smem_u32(&bar_aux), C::STAGING);
+#pragma unroll
+        for (int h = 0; h < BN / 64; ++h) tma_load_3d(sOut + h * (BM * 128), &mapAux, smem_u32(&bar_aux), n0 + 64 * h, m0, bz);
+      }
+      }
     }
   } else if (warp == 1) {
     constexpr uint32_t idesc = make_idesc_bf16(BM, BN, A_MN != 0, B_MN != 0);
@@ -162,31 +177,45 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     // MN-major: [64 k-rows][128 bytes] atoms of 64 M/N elements, 8192 bytes apart; 16 k-rows = 2048 bytes per k-step.
     const uint64_t dA = A_MN ? make_smem_desc<128>(sA, 64 * 128, 1024) : make_smem_desc<128>(sA, 16, 1024);
     const uint64_t dB = B_MN ? make_smem_desc<128>(sB, 64 * 128, 1024) : make_smem_desc<128>(sB, 16, 1024);
-    uint32_t t = 0;
-    for (int kb = kb0; kb < kb1; ++kb, ++t) {
-      const uint32_t st = t % ST;
-      mbar_wait(smem_u32(&bar_full[st]), (t / ST) & 1);
-      tc_fence_after();
-      const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
+    uint32_t t = 0, it = 0;
+    for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
+      const uint32_t ab = it & 1, acc = tmem + ab * BN;
+      if (it > 1) {   // the epilogue has read this accumulator's previous tile out of TMEM
+        mbar_wait(smem_u32(&bar_acc_free[ab]), ((it >> 1) - 1) & 1);
+        tc_fence_after();
+      }
+      for (int kb = kb0; kb < kb1; ++kb, ++t) {
+        const uint32_t st = t % ST;
+        mbar_wait(smem_u32(&bar_full[st]), (t / ST) & 1);
+        tc_fence_after();
+        const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
 #pragma unroll
-      for (int kk = 0; kk < BK / 16; ++kk)
-        mma_ss_e(tmem, a + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc, (t > 0 || kk > 0) ? 1u : 0u);
-      tc_commit_e(smem_u32(&bar_empty[st]));
+        for (int kk = 0; kk < BK / 16; ++kk)
+          mma_ss_e(acc, a + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc,
+                   (kb > kb0 || kk > 0) ? 1u : 0u);
+        tc_commit_e(smem_u32(&bar_empty[st]));
+      }
+      tc_commit_e(smem_u32(&bar_acc[ab]));
     }
-    tc_commit_e(smem_u32(&bar_acc));
   } else {
     // ------------------------------------------------------------------------------ epilogue
     const int q = warp & 3, r = 32 * q + lane;
     const int c_lo = ((warp - 2) >> 2) * (BN / 64), c_hi = c_lo + BN / 64;   // this warp's 32-column groups
-    const int m = m0 + r;
-    const uint32_t tacc = tmem + ((uint32_t)(32 * q) << 16);
-    float rs = p.alpha;
-    if (p.row_scale && m < p.M) rs *= __ldg(p.row_scale + (size_t)bz * p.M + m);
-    mbar_wait(smem_u32(&bar_acc), 0);
-    tc_fence_after();
-    if (p.aux_mode != AUX_NONE) mbar_wait(smem_u32(&bar_aux), 0);
+    const uint32_t tacc0 = tmem + ((uint32_t)(32 * q) << 16);
     const bool has_k = kb1 > kb0;
     const int passes = p.dual_out ? 2 : 1;
+    uint32_t it = 0;
+    for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
+    const int m0 = my * BM, m = m0 + r;
+    float rs = p.alpha;
+    if (p.row_scale && m < p.M) rs *= __ldg(p.row_scale + (size_t)bz * p.M + m);
+    const uint32_t ab = it & 1, tacc = tacc0 + ab * BN;
+    mbar_wait(smem_u32(&bar_acc[ab]), (it >> 1) & 1);
+    tc_fence_after();
+    // the staging tile: free once the previous tile's store has read it (with an auxiliary tile the producer waited
+    // for that before loading it)
+    if (p.aux_mode != AUX_NONE) mbar_wait(smem_u32(&bar_aux), it & 1);
+    else if (it > 0 && !splitk) mbar_wait(smem_u32(&bar_out_free), (it - 1) & 1);
     for (int pass = 0; pass < passes; ++pass) {
       // dual output: pass 0 stores the value before the activation (C0), pass 1 the value after it (C1)
       const bool do_act = p.act == ACT_GELU && (!p.dual_out || pass == 1);
@@ -239,6 +268,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           sts_v4(off, o.x, o.y, o.z, o.w);
         }
       }
+      if (pass == passes - 1 || splitk) {   // the accumulator has been read for the last time
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free[ab]));
+      }
       if (splitk) break;
       fence_proxy_async_smem();
       named_bar_sync(1, kEpiWarps * 32);
@@ -254,15 +288,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           tma_store_3d(mc, sOut + h * (BM * 128), cin, m0, bz);
         }
         bulk_commit();
-        bulk_wait<0>();
+        bulk_wait_read<0>();   // (the staging tile has been read; the writes themselves complete in the background)
       }
       // (dual output: the staging tile is rewritten by the next pass only after the store has read it)
       if (passes > 1) named_bar_sync(1, kEpiWarps * 32);
     }
+    // next tile: the producer may overwrite the staging tile (the store above has completed), and through it -- its
+    // loads precede the MMAs that precede bar_acc -- so may the other epilogue warps
+    if (warp == 2 && lane == 0) mbar_arrive(smem_u32(&bar_out_free));
+    }
+    if (warp == 2 && lane == 0) bulk_wait<0>();   // the CTA's stores are complete before it exits
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, BN);
+  if (warp == 1) tmem_dealloc(tmem, 2 * BN);
 }
 
 __global__ void reduce_slabs_kernel(const float* __restrict__ partial, int slabs, long long mn, float scale,
@@ -341,8 +380,13 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   static SmemAttr attr;
   cudaError_t e = attr.ensure(kern, Cfg<BN>::SMEM_AUX, di->ordinal);
   if (e != cudaSuccess) return e;
-  const int smem = p.aux_mode != AUX_NONE ? Cfg<BN>::SMEM_AUX : Cfg<BN>::SMEM_MAIN;
-  dim3 grid((p.N + BN - 1) / BN, (p.M + BM - 1) / BM, p.partial ? kp.slabs : p.batch);
+  const int smem = Cfg<BN>::SMEM_AUX;
+  // row tiles per launch: all of them (split-K, batched and small problems), else as many as keep every CTA resident
+  // (three per SM); each CTA then walks its column of row tiles (see the kernel)
+  const int tiles_n = (p.N + BN - 1) / BN, tiles_m = (p.M + BM - 1) / BM, gz = p.partial ? kp.slabs : p.batch;
+  int gy = tiles_m;
+  if (!p.partial) gy = std::min(tiles_m, std::max(1, (2 * di->num_sms) / (tiles_n * gz)));
+  dim3 grid(tiles_n, gy, gz);
   kern<<<grid, kThreads, smem, stream>>>(ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
   count_launch();
   return cudaGetLastError();
