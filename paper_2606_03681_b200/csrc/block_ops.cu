@@ -256,7 +256,8 @@ cudaError_t weight_grad(const void* dY, long long ldy, const void* A, long long 
   p.A = {dY, 1, ldy, 0};
   p.B = {A, 1, lda, 0};
   p.alpha = 1.f;
-  const int tiles = ((N + 127) / 128) * ((K + 63) / 64);
+  // (column tiles: 256 wide when K allows it, else 128 / 64 -- gemm::launch)
+  const int tiles = ((N + 127) / 128) * (K % 256 == 0 ? K / 256 : (K + 63) / 64);
   p.slabs = gemm::slabs_for(M, tiles, di->num_sms);
   if ((size_t)p.slabs * N * K > ws_floats) return cudaErrorInvalidValue;
   p.partial = ws_f32;

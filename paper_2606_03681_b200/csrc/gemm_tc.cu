@@ -85,6 +85,7 @@ struct Cfg {
   // the epilogue's staging tile is a buffer of its own (an auxiliary tile is prefetched into it when there is one):
   // the ring keeps loading the next tile while the epilogue of the current one writes it
   static constexpr int SMEM_AUX = ST * STAGE + STAGING + 1024;
+  static constexpr int SMEM_SPLITK = ST * STAGE + 1024;   // (fp32 partial tiles go straight to global memory)
 };
 
 template <int BN, int A_MN, int B_MN>
@@ -112,7 +113,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   const int bz = splitk ? 0 : blockIdx.z, slab = splitk ? blockIdx.z : 0;
   const int kb0 = slab * p.kb_per_slab, kb1 = min(p.kb_total, kb0 + p.kb_per_slab);
 
-  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), 2 * BN);   // two accumulators: tile i's epilogue under tile i+1's MMAs
+  // two accumulators (tile i's epilogue under tile i+1's MMAs); a split-K CTA computes one tile and needs one
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), splitk ? BN : 2 * BN);
   if (threadIdx.x == 0) {
     for (int i = 0; i < ST; ++i) {
       mbar_init(smem_u32(&bar_full[i]), 1);
@@ -301,7 +303,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 2 * BN);
+  if (warp == 1) tmem_dealloc(tmem, splitk ? BN : 2 * BN);
 }
 
 __global__ void reduce_slabs_kernel(const float* __restrict__ partial, int slabs, long long mn, float scale,
@@ -378,9 +380,10 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   if (!ok) return cudaErrorInvalidValue;
   auto kern = gemm_tc_kernel<BN, A_MN, B_MN>;
   static SmemAttr attr;
-  cudaError_t e = attr.ensure(kern, Cfg<BN>::SMEM_AUX, di->ordinal);
+  cudaError_t e = attr.ensure(kern, BN > 128 ? Cfg<BN>::SMEM_SPLITK : Cfg<BN>::SMEM_AUX, di->ordinal);
   if (e != cudaSuccess) return e;
-  const int smem = Cfg<BN>::SMEM_AUX;
+  if (BN > 128 && !p.partial) return cudaErrorInvalidValue;   // (256-wide tiles: split-K only)
+  const int smem = p.partial ? Cfg<BN>::SMEM_SPLITK : Cfg<BN>::SMEM_AUX;
   // row tiles per launch: all of them (split-K, batched and small problems), else as many as keep every CTA resident
   // (three per SM); each CTA then walks its column of row tiles (see the kernel)
   const int tiles_n = (p.N + BN - 1) / BN, tiles_m = (p.M + BM - 1) / BM, gz = p.partial ? kp.slabs : p.batch;
@@ -433,6 +436,10 @@ cudaError_t launch(const Problem& p, cudaStream_t stream) {
   if (p.a_split_k > 0 && (p.a_split_k % 64 != 0 || p.K != 3 * p.a_split_k || !p.A2 || !p.A3)) return cudaErrorInvalidValue;
   if (p.dual_out && (p.split_cols > 0 || p.partial)) return cudaErrorInvalidValue;
   // 128-wide tiles when N allows it (fewer re-reads of A), else 64; split outputs need 64-column granularity
+  // Split-K weight gradients (both operands MN-major, K = all cells): these are bound by the operand traffic from L2
+  // (~8 TB/s measured with 128 x 128 tiles, each operand byte fetched by two to six CTAs), so the tile is as wide as
+  // the MMA allows
+  if (p.partial && p.A.mn_major && p.B.mn_major && p.N % 256 == 0) return launch_t<256, 1, 1>(p, kp, stream);
   const bool bn128 = (p.N % 128 == 0) && (p.split_cols == 0 || p.split_cols % 128 == 0);
   return bn128 ? launch_bn<128>(p, kp, stream) : launch_bn<64>(p, kp, stream);
 }
