@@ -249,11 +249,14 @@ gemm::Problem nn(const void* dY, long long M, int N, const void* W, int K, void*
 }
 
 // dW[N][K] (fp32) = dY[M][N]^T A[M][K], reduced over the M cells in split-K slabs (partials in ws_f32)
+// (dY2, dY3 != nullptr: dY is three tensors of N / 3 columns each, stacked along N -- the rows of dW)
 cudaError_t weight_grad(const void* dY, long long ldy, const void* A, long long lda, long long M, int N, int K,
-                        float* dW, float* ws_f32, size_t ws_floats, const DeviceInfo* di, cudaStream_t stream) {
+                        float* dW, float* ws_f32, size_t ws_floats, const DeviceInfo* di, cudaStream_t stream,
+                        const void* dY2 = nullptr, const void* dY3 = nullptr) {
   gemm::Problem p{};
   p.M = N; p.N = K; p.K = (int)M; p.batch = 1;
   p.A = {dY, 1, ldy, 0};
+  if (dY2) { p.A2 = dY2; p.A3 = dY3; p.a_split_m = N / 3; }
   p.B = {A, 1, lda, 0};
   p.alpha = 1.f;
   // (column tiles: 256 wide when K allows it, else 128 / 64 -- gemm::launch)
@@ -363,7 +366,7 @@ size_t attn_block_bwd_ws_bytes(const Shape& s, int axis, int num_sms) {
   size_t n = (size_t)cells * e * 2 * 5;
   n += axis == 0 ? feature_workspace_bytes(s) : item_bwd_workspace_bytes(s);
   n = (n + 255) & ~(size_t)255;
-  n += (size_t)130 * e * e * sizeof(float) + (size_t)num_sms * 8 * e * sizeof(float) + 1024;
+  n += (size_t)130 * 3 * e * e * sizeof(float) + (size_t)num_sms * 8 * e * sizeof(float) + 1024;   // (dWqkv partials)
   return n;
 }
 
@@ -385,7 +388,7 @@ cudaError_t launch_attn_block_bwd(const Shape& s, int axis, float alpha, const v
   off += axis == 0 ? feature_workspace_bytes(s) : item_bwd_workspace_bytes(s);
   off = (off + 255) & ~(size_t)255;
   float* partial = reinterpret_cast<float*>(w + off);
-  const size_t partial_floats = (size_t)130 * e * e;
+  const size_t partial_floats = (size_t)130 * 3 * e * e;
   float* dg_partial = partial + partial_floats;
   // do = dy Wo ; dWo[e][e] = dy^T o
   gemm::Problem p = nn(dy, cells, e, Wo, e, d_o);
@@ -397,11 +400,16 @@ cudaError_t launch_attn_block_bwd(const Shape& s, int axis, float alpha, const v
                  : launch_item_bwd(s, q, k, v, o, d_o, lse, dq, dk, dv, static_cast<float*>(attn_ws), stream);
   if (er != cudaSuccess) return er;
   // dWqkv[3e][e]: three [e][e] blocks  d{q,k,v}^T h
-  const void* grads[3] = {dq, dk, dv};
-  for (int t = 0; t < 3; ++t)
-    if ((er = weight_grad(grads[t], e, h, e, cells, e, e, dWqkv + (size_t)t * e * e, partial, partial_floats, di,
-                          stream)) != cudaSuccess)
+  if (e % 128 == 0) {   // one launch over the three gradients: h is read once
+    if ((er = weight_grad(dq, e, h, e, cells, 3 * e, e, dWqkv, partial, partial_floats, di, stream, dk, dv)) != cudaSuccess)
       return er;
+  } else {
+    const void* grads[3] = {dq, dk, dv};
+    for (int t = 0; t < 3; ++t)
+      if ((er = weight_grad(grads[t], e, h, e, cells, e, e, dWqkv + (size_t)t * e * e, partial, partial_floats, di,
+                            stream)) != cudaSuccess)
+        return er;
+  }
   // dh = [dq | dk | dv] Wqkv   (A split over the three tensors along K)
   gemm::Problem r = linear_problem(cells, e, 3 * e);
   r.A = {dq, 0, e, 0};

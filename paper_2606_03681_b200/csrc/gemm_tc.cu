@@ -37,6 +37,7 @@ struct KParams {
   int split_cols;
   int a_batched, b_batched;   // 0: operand shared by all batches (TMA batch coordinate 0)
   int a_split_k;              // > 0: A is three tensors of this many columns
+  int a_split_m;              // > 0: (MN-major A) three tensors of this many output rows
   int dual_out;
 };
 
@@ -149,8 +150,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         mbar_arrive_expect_tx(full, C::STAGE);
         const uint32_t a = sA + st * A_BYTES, b = sB + st * C::B_BYTES;
         if (A_MN) {
-          tma_load_3d(a, &mapA, full, m0, kb * BK, ba);
-          tma_load_3d(a + 64 * 128, &mapA, full, m0 + 64, kb * BK, ba);
+          const CUtensorMap* ma = &mapA;
+          int ml = m0;
+          if (p.a_split_m > 0) {
+            const int seg = m0 / p.a_split_m;
+            ml = m0 - seg * p.a_split_m;
+            ma = seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3);
+          }
+          tma_load_3d(a, ma, full, ml, kb * BK, ba);
+          tma_load_3d(a + 64 * 128, ma, full, ml + 64, kb * BK, ba);
         } else if (p.a_split_k > 0) {
           const int seg = (kb * BK) / p.a_split_k, kin = kb * BK - seg * p.a_split_k;
           tma_load_3d(a, seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3), full, kin, m0, ba);
@@ -362,6 +370,11 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   bool ok = p.A.mn_major ? make_map(&ma, p.A.ptr, p.M, p.K, p.A.ld, p.batch, p.A.batch_stride, 64)
                          : make_map(&ma, p.A.ptr, p.K, p.M, p.A.ld, p.batch, p.A.batch_stride, BM);
   ma2 = ma; ma3 = ma;
+  if (p.a_split_m > 0) {
+    ok = ok && p.A.mn_major && make_map(&ma, p.A.ptr, p.a_split_m, p.K, p.A.ld, p.batch, p.A.batch_stride, 64) &&
+         make_map(&ma2, p.A2, p.a_split_m, p.K, p.A.ld, p.batch, p.A.batch_stride, 64) &&
+         make_map(&ma3, p.A3, p.a_split_m, p.K, p.A.ld, p.batch, p.A.batch_stride, 64);
+  }
   if (p.a_split_k > 0) {
     ok = ok && !p.A.mn_major && make_map(&ma, p.A.ptr, p.a_split_k, p.M, p.A.ld, p.batch, p.A.batch_stride, BM) &&
          make_map(&ma2, p.A2, p.a_split_k, p.M, p.A.ld, p.batch, p.A.batch_stride, BM) &&
@@ -432,7 +445,9 @@ cudaError_t launch(const Problem& p, cudaStream_t stream) {
   kp.alpha = p.alpha; kp.beta = p.beta; kp.row_scale = p.row_scale; kp.act = p.act; kp.aux_mode = p.aux_mode;
   kp.partial = p.partial; kp.split_cols = p.split_cols;
   kp.a_batched = p.A.batch_stride != 0; kp.b_batched = p.B.batch_stride != 0;
-  kp.a_split_k = p.a_split_k; kp.dual_out = p.dual_out;
+  kp.a_split_k = p.a_split_k; kp.a_split_m = p.a_split_m; kp.dual_out = p.dual_out;
+  if (p.a_split_m > 0 && (p.a_split_m % 128 != 0 || p.M != 3 * p.a_split_m || !p.A2 || !p.A3 || !p.A.mn_major || p.a_split_k > 0))
+    return cudaErrorInvalidValue;
   if (p.a_split_k > 0 && (p.a_split_k % 64 != 0 || p.K != 3 * p.a_split_k || !p.A2 || !p.A3)) return cudaErrorInvalidValue;
   if (p.dual_out && (p.split_cols > 0 || p.partial)) return cudaErrorInvalidValue;
   // 128-wide tiles when N allows it (fewer re-reads of A), else 64; split outputs need 64-column granularity

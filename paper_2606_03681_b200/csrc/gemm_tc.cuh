@@ -40,6 +40,9 @@ struct Problem {
   const void* A2;
   const void* A3;
   int a_split_k;
+  // MN-major A split along M over three tensors of a_split_m rows of the output each (dWqkv = [dq | dk | dv]^T h in
+  // one launch): A.ptr, A2, A3 with A's pitch; 0 = one tensor.  a_split_m % 128 == 0, M == 3 a_split_m.
+  int a_split_m;
   // output: bf16 [M][ldc] per batch, optionally split over tensors of split_cols columns
   void* C[3];
   long long ldc, c_batch_stride;
