@@ -77,6 +77,7 @@ ATTN_CASES = [
     ("e64", 2, 70, 5, 2, 32, 40, "none", 1.0),
     ("e192_masked", 2, 150, 12, 6, 32, 100, "prefix", 0.95),
     ("e256", 1, 300, 6, 4, 64, 200, "none", 0.95 ** 4),
+    ("e128", 1, 130, 3, 4, 32, 90, "none", 1.0),   # dWqkv in one launch, one 128-row tile per gradient tensor
 ]
 
 
