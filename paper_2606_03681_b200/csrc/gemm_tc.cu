@@ -115,6 +115,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   const int kb0 = slab * p.kb_per_slab, kb1 = min(p.kb_total, kb0 + p.kb_per_slab);
 
   // two accumulators (tile i's epilogue under tile i+1's MMAs); a split-K CTA computes one tile and needs one
+  // Programmatic dependent launch: the next GEMM of the stream may bring its CTAs up (TMEM allocation, barrier set-up)
+  // while this one runs, and this one did the same under its predecessor; nothing below the griddepcontrol.wait
+  // touches global memory before the predecessor has completed and flushed.  (Chains of small GEMMs -- the 16
+  // launches of Newton-Schulz -- are latency-bound: ~7 us per kernel.)
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), splitk ? BN : 2 * BN);
   if (threadIdx.x == 0) {
     for (int i = 0; i < ST; ++i) {
@@ -133,6 +138,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   if (warp == 0) {
     if (lane == 0) {
@@ -403,9 +409,19 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   int gy = tiles_m;
   if (!p.partial) gy = std::min(tiles_m, std::max(1, (2 * di->num_sms) / (tiles_n * gz)));
   dim3 grid(tiles_n, gy, gz);
-  kern<<<grid, kThreads, smem, stream>>>(ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr_pdl{};
+  attr_pdl.id = cudaLaunchAttributeProgrammaticStreamSerialization;   // (see griddepcontrol in the kernel)
+  attr_pdl.val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = &attr_pdl;
+  cfg.numAttrs = 1;
+  e = cudaLaunchKernelEx(&cfg, kern, ma, ma2, ma3, mb, maux, mc[0], mc[1], mc[2], kp);
   count_launch();
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 template <int BN>
