@@ -157,7 +157,7 @@ __host__ __device__ constexpr bool pair_is_poly(int k) {
   }
 // TR_INIT() once per kernel (reads the buffer pointer into a register: a stamp must not wait for a global load;
 // measured ~200 clk per stamp with the load, which distorted what it timed)
-#define TR_INIT() long long* const tr_buf_ = blockIdx.x == 0 ? g_trace : nullptr
+#define TR_INIT() long long* const tr_buf_ = (blockIdx.x | blockIdx.y | blockIdx.z) == 0 ? g_trace : nullptr
 #define TR(ev, tile) \
   do { if (tr_buf_ && (tile) < 64) tr_buf_[(tile) * 16 + (ev)] = clock64(); } while (0)
 #else

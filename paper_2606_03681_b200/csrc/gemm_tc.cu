@@ -18,6 +18,8 @@
 namespace tabattn {
 namespace gemm {
 
+TABATTN_TRACE_DEFINE(tabattn_debug_set_trace_gemm)
+
 namespace {
 
 using namespace tc;
@@ -54,27 +56,42 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src,
                : "memory");
 }
 
-// erf by Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7, far below the bf16 step of the outputs): one reciprocal, one
-// ex2 and five FMAs instead of erff's ~30 instructions -- the epilogue of the MLP GEMMs is bound by this arithmetic.
-// Returns erf(x / sqrt 2) and leaves exp(-x^2 / 2) in `ex` (the Gaussian factor of gelu').
-__device__ __forceinline__ float erf_half(float x, float& ex) {
-  const float z = fabsf(x) * 0.70710678118654752f;
-  const float t = __frcp_rn(fmaf(0.3275911f, z, 1.f));
-  ex = fast_exp2(-z * z * kLog2e);
-  float p = fmaf(t, 1.061405429f, -1.453152027f);
-  p = fmaf(p, t, 1.421413741f);
-  p = fmaf(p, t, -0.284496736f);
-  p = fmaf(p, t, 0.254829592f);
-  return copysignf(fmaf(-p * t, ex, 1.f), x);
+// GELU (exact, erf form) in the epilogues.  The MLP up-projection's epilogue was bound by this arithmetic: the timeline
+// (profiles/r02_blocks.md) shows 9,800 of a tile's 16,000 clocks in the GELU pass, ~39 issue slots per element with
+// erf by Abramowitz & Stegun (a reciprocal, an ex2 and ten scalar FMAs per element).  Now erf(x / sqrt 2) is evaluated
+// for two values at a time on the FMA pipe alone: z = x / sqrt 2 clamped to [-3, 3] (erf(3) = 1 - 2.2e-5), then
+// z P(z^2) with a degree-8 polynomial fitted at Chebyshev nodes of z^2 in [0, 9].  |erf error| <= 4.2e-5 in fp32,
+// |gelu error| <= 8.8e-5 (x in [-6, 6], checked on 200,001 points against math.erf): 1/20 of the bf16 rounding step of
+// an activation of size 1, absolute -- the far negative tail, where gelu itself is below 4e-3, is only that accurate.
+__device__ __forceinline__ uint64_t pk2(float c) { return f2pack(c, c); }
+__device__ __forceinline__ uint64_t erf_half2(uint64_t x) {
+  float a, b;
+  f2unpack(mul2(x, pk2(0.70710678118654752f)), a, b);
+  a = fminf(fmaxf(a, -3.f), 3.f);
+  b = fminf(fmaxf(b, -3.f), 3.f);
+  const uint64_t z = f2pack(a, b), s = mul2(z, z);
+  uint64_t p = fma2(pk2(4.918276073e-08f), s, pk2(-2.267730623e-06f));
+  p = fma2(p, s, pk2(4.614729186e-05f));
+  p = fma2(p, s, pk2(-5.535572417e-04f));
+  p = fma2(p, s, pk2(4.437862287e-03f));
+  p = fma2(p, s, pk2(-2.564961361e-02f));
+  p = fma2(p, s, pk2(1.118625027e-01f));
+  p = fma2(p, s, pk2(-3.758186012e-01f));
+  p = fma2(p, s, pk2(1.128362939e+00f));
+  return mul2(z, p);
 }
-__device__ __forceinline__ float gelu_f(float x) {
-  float ex;
-  return 0.5f * x * (1.f + erf_half(x, ex));
+// gelu(x) = x/2 + x/2 erf(x / sqrt 2) for a pair
+__device__ __forceinline__ void gelu_pair(float& x0, float& x1) {
+  const uint64_t x = f2pack(x0, x1), h = mul2(x, pk2(0.5f));
+  f2unpack(fma2(h, erf_half2(x), h), x0, x1);
 }
-__device__ __forceinline__ float gelu_grad_f(float x) {
-  float ex;
-  const float er = erf_half(x, ex);
-  return fmaf(x * 0.3989422804014327f, ex, 0.5f * (1.f + er));
+// gelu'(x) = 1/2 + 1/2 erf(x / sqrt 2) + x exp(-x^2 / 2) / sqrt(2 pi) for a pair (the Gaussian on the MUFU)
+__device__ __forceinline__ void gelu_grad_pair(float x0, float x1, float& g0, float& g1) {
+  const uint64_t x = f2pack(x0, x1);
+  float e0, e1;
+  f2unpack(mul2(mul2(x, x), pk2(-0.5f * kLog2e)), e0, e1);
+  const uint64_t gauss = mul2(mul2(x, pk2(0.3989422804014327f)), f2pack(fast_exp2(e0), fast_exp2(e1)));
+  f2unpack(add2(fma2(erf_half2(x), pk2(0.5f), pk2(0.5f)), gauss), g0, g1);
 }
 
 template <int BN>
@@ -96,8 +113,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
                const __grid_constant__ CUtensorMap mapAux, const __grid_constant__ CUtensorMap mapC0,
                const __grid_constant__ CUtensorMap mapC1, const __grid_constant__ CUtensorMap mapC2,
                const __grid_constant__ KParams p) {
+  TR_INIT();
   using C = Cfg<BN>;
   constexpr int ST = C::ST;
+  // (trace builds: only the projections with split or dual outputs -- the QKV and the MLP up-projection -- are stamped)
+  [[maybe_unused]] const bool traced = p.split_cols > 0 || p.dual_out;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sA = sbase, sB = sA + ST * A_BYTES;
@@ -153,6 +173,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       for (int kb = kb0; kb < kb1; ++kb, ++t) {
         const uint32_t st = t % ST, full = smem_u32(&bar_full[st]);
         mbar_wait<true>(smem_u32(&bar_empty[st]), ((t / ST) & 1) ^ 1);
+        if (traced && kb == kb0) TR(0, it);                 // first stage of the tile free, loads start
         mbar_arrive_expect_tx(full, C::STAGE);
         const uint32_t a = sA + st * A_BYTES, b = sB + st * C::B_BYTES;
         if (A_MN) {
@@ -178,6 +199,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           tma_load_3d(b, &mapB, full, kb * BK, n0, bb);
         }
       }
+      if (traced) TR(1, it);                                // last load of the tile issued
       if (p.aux_mode != AUX_NONE) {
         // the tile of the auxiliary operand lands in the staging tile the epilogue later overwrites in place
         if (it > 0) mbar_wait<true>(smem_u32(&bar_out_free), (it - 1) & 1);
@@ -203,6 +225,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       for (int kb = kb0; kb < kb1; ++kb, ++t) {
         const uint32_t st = t % ST;
         mbar_wait(smem_u32(&bar_full[st]), (t / ST) & 1);
+        if (traced && lane == 0 && kb == kb0) TR(2, it);    // first k-block landed
         tc_fence_after();
         const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
 #pragma unroll
@@ -212,6 +235,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         tc_commit_e(smem_u32(&bar_empty[st]));
       }
       tc_commit_e(smem_u32(&bar_acc[ab]));
+      if (traced && lane == 0) TR(3, it);                   // MMAs of the tile issued
     }
   } else {
     // ------------------------------------------------------------------------------ epilogue
@@ -227,6 +251,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     if (p.row_scale && m < p.M) rs *= __ldg(p.row_scale + (size_t)bz * p.M + m);
     const uint32_t ab = it & 1, tacc = tacc0 + ab * BN;
     mbar_wait(smem_u32(&bar_acc[ab]), (it >> 1) & 1);
+    if (traced && threadIdx.x == 64) TR(4, it);             // accumulator complete
     tc_fence_after();
     // the staging tile: free once the previous tile's store has read it (with an auxiliary tile the producer waited
     // for that before loading it)
@@ -274,11 +299,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           }
           if (do_act) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = gelu_f(f[e]);
+            for (int e = 0; e < 8; e += 2) gelu_pair(f[e], f[e + 1]);
           }
           if (p.aux_mode == AUX_GELU_GRAD) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] *= gelu_grad_f(a[e]);
+            for (int e = 0; e < 8; e += 2) {
+              float g0, g1;
+              gelu_grad_pair(a[e], a[e + 1], g0, g1);
+              f[e] *= g0;
+              f[e + 1] *= g1;
+            }
           }
           const uint4 o = pack8(f);
           sts_v4(off, o.x, o.y, o.z, o.w);
@@ -290,8 +320,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free[ab]));
       }
       if (splitk) break;
+      if (traced && threadIdx.x == 64) TR(5 + 4 * pass, it);  // this warp's part of the staging tile written
       fence_proxy_async_smem();
       named_bar_sync(1, kEpiWarps * 32);
+      if (traced && threadIdx.x == 64) TR(6 + 4 * pass, it);  // all epilogue warps done
       if (warp == 2 && lane == 0) {
 #pragma unroll
         for (int h = 0; h < BN / 64; ++h) {
@@ -304,7 +336,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           tma_store_3d(mc, sOut + h * (BM * 128), cin, m0, bz);
         }
         bulk_commit();
+        if (traced) TR(7 + 4 * pass, it);                   // store issued
         bulk_wait_read<0>();   // (the staging tile has been read; the writes themselves complete in the background)
+        if (traced) TR(8 + 4 * pass, it);                   // staging tile read by the store
       }
       // (dual output: the staging tile is rewritten by the next pass only after the store has read it)
       if (passes > 1) named_bar_sync(1, kEpiWarps * 32);
