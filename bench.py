@@ -469,7 +469,7 @@ def time_next_rows(torch, tab, dev, peaks, iters=20):
     out["newton_schulz"] = {"nb": nb, "m": m, "n": m, "steps": 5, "ms": tns, "TFLOP/s": fl / tns / 1e9,
                             "graph_ms": tng, "graph_TFLOP/s": fl / tng / 1e9,
                             "launches": 16, "note": "30 matrices of 256x256 (3.9 MB): L2-resident and launch-bound"}
-    out["tiny_layer"] = time_tiny_layer(torch, tab, dev)
+    out["tiny_layer"] = time_tiny_layer(torch, tab, dev, iters=50 * iters)
     return out
 
 
