@@ -41,6 +41,9 @@ struct KParams {
   int a_split_k;              // > 0: A is three tensors of this many columns
   int a_split_m;              // > 0: (MN-major A) three tensors of this many output rows
   int dual_out;
+  // direct epilogue (no auxiliary tile, not split-K): the outputs as raw pointers
+  unsigned char* c_ptr[3];
+  long long ldc, c_bstride;   // elements
 };
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2) {
@@ -97,13 +100,18 @@ __device__ __forceinline__ void gelu_grad_pair(float x0, float x1, float& g0, fl
 template <int BN>
 struct Cfg {
   static constexpr int ST = BN == 64 ? 3 : 2;
+  // ring depth when the epilogue needs no staging tile (it stores straight from registers): the freed shared memory
+  // holds one more stage -- the plain projections are bound by the latency of their operand loads (timeline,
+  // profiles/r02_blocks.md: a round trip is ~2,400 clk and a K = 768 tile was six of them)
+  static constexpr int ST_DIRECT = ST + 1, ST_MAX = ST_DIRECT;
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE = A_BYTES + B_BYTES;
   static constexpr int STAGING = (BN / 64) * (BM * 128);
   // the epilogue's staging tile is a buffer of its own (an auxiliary tile is prefetched into it when there is one):
   // the ring keeps loading the next tile while the epilogue of the current one writes it
   static constexpr int SMEM_AUX = ST * STAGE + STAGING + 1024;
-  static constexpr int SMEM_SPLITK = ST * STAGE + 1024;   // (fp32 partial tiles go straight to global memory)
+  static constexpr int SMEM_SPLITK = ST * STAGE + 1024;
+  static constexpr int SMEM_DIRECT = ST_DIRECT * STAGE + 1024;   // (fp32 partial tiles go straight to global memory)
 };
 
 template <int BN, int A_MN, int B_MN>
@@ -120,9 +128,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   [[maybe_unused]] const bool traced = p.split_cols > 0 || p.dual_out;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sA = sbase, sB = sA + ST * A_BYTES;
-  const uint32_t sOut = sB + ST * C::B_BYTES;   // the epilogue's staging tile (the auxiliary tile lands in it first)
-  __shared__ uint64_t bar_full[ST], bar_empty[ST], bar_acc[2], bar_aux, bar_acc_free[2], bar_out_free;
+  const bool direct = BN <= 128 && p.aux_mode == AUX_NONE && p.partial == nullptr;
+  const uint32_t st_n = direct ? C::ST_DIRECT : ST;          // ring depth
+  const uint32_t sA = sbase, sB = sA + st_n * A_BYTES;
+  const uint32_t sOut = sB + st_n * C::B_BYTES;   // the epilogue's staging tile (the auxiliary tile lands in it first)
+  __shared__ uint64_t bar_full[C::ST_MAX], bar_empty[C::ST_MAX], bar_acc[2], bar_aux, bar_acc_free[2], bar_out_free;
   __shared__ uint32_t tmem_slot;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
@@ -142,7 +152,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), splitk ? BN : 2 * BN);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < ST; ++i) {
+    for (int i = 0; i < C::ST_MAX; ++i) {
       mbar_init(smem_u32(&bar_full[i]), 1);
       mbar_init(smem_u32(&bar_empty[i]), 1);
     }
@@ -165,14 +175,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       tma_prefetch_desc(&mapA);
       tma_prefetch_desc(&mapB);
       const int ba = p.a_batched ? bz : 0, bb = p.b_batched ? bz : 0;
-      uint32_t t = 0, it = 0;
+      uint32_t st = 0, ph = 0, it = 0;
       for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
       const int m0 = my * BM;
       // (the A / B loads of a tile run ahead under the previous tile's epilogue; the auxiliary load, below, waits for
       // the staging tile)
-      for (int kb = kb0; kb < kb1; ++kb, ++t) {
-        const uint32_t st = t % ST, full = smem_u32(&bar_full[st]);
-        mbar_wait<true>(smem_u32(&bar_empty[st]), ((t / ST) & 1) ^ 1);
+      for (int kb = kb0; kb < kb1; ++kb) {
+        const uint32_t full = smem_u32(&bar_full[st]);
+        mbar_wait<true>(smem_u32(&bar_empty[st]), ph ^ 1);
         if (traced && kb == kb0) TR(0, it);                 // first stage of the tile free, loads start
         mbar_arrive_expect_tx(full, C::STAGE);
         const uint32_t a = sA + st * A_BYTES, b = sB + st * C::B_BYTES;
@@ -198,6 +208,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         } else {
           tma_load_3d(b, &mapB, full, kb * BK, n0, bb);
         }
+        if (++st == st_n) { st = 0; ph ^= 1; }
       }
       if (traced) TR(1, it);                                // last load of the tile issued
       if (p.aux_mode != AUX_NONE) {
@@ -215,16 +226,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     // MN-major: [64 k-rows][128 bytes] atoms of 64 M/N elements, 8192 bytes apart; 16 k-rows = 2048 bytes per k-step.
     const uint64_t dA = A_MN ? make_smem_desc<128>(sA, 64 * 128, 1024) : make_smem_desc<128>(sA, 16, 1024);
     const uint64_t dB = B_MN ? make_smem_desc<128>(sB, 64 * 128, 1024) : make_smem_desc<128>(sB, 16, 1024);
-    uint32_t t = 0, it = 0;
+    uint32_t st = 0, ph = 0, it = 0;
     for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
       const uint32_t ab = it & 1, acc = tmem + ab * BN;
       if (it > 1) {   // the epilogue has read this accumulator's previous tile out of TMEM
         mbar_wait(smem_u32(&bar_acc_free[ab]), ((it >> 1) - 1) & 1);
         tc_fence_after();
       }
-      for (int kb = kb0; kb < kb1; ++kb, ++t) {
-        const uint32_t st = t % ST;
-        mbar_wait(smem_u32(&bar_full[st]), (t / ST) & 1);
+      for (int kb = kb0; kb < kb1; ++kb) {
+        mbar_wait(smem_u32(&bar_full[st]), ph);
         if (traced && lane == 0 && kb == kb0) TR(2, it);    // first k-block landed
         tc_fence_after();
         const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
@@ -233,6 +243,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           mma_ss_e(acc, a + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc,
                    (kb > kb0 || kk > 0) ? 1u : 0u);
         tc_commit_e(smem_u32(&bar_empty[st]));
+        if (++st == st_n) { st = 0; ph ^= 1; }
       }
       tc_commit_e(smem_u32(&bar_acc[ab]));
       if (traced && lane == 0) TR(3, it);                   // MMAs of the tile issued
@@ -253,6 +264,50 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     mbar_wait(smem_u32(&bar_acc[ab]), (it >> 1) & 1);
     if (traced && threadIdx.x == 64) TR(4, it);             // accumulator complete
     tc_fence_after();
+    if (direct) {
+      // no staging tile: a quad of lanes transposes its four rows' 64-byte groups in registers and stores one row per
+      // instruction (quad_transpose, common.cuh); no fence, CTA barrier or store wait in the tile's path
+      if constexpr (BN <= 128) {
+        QuadRows qr;
+        qr.init((size_t)m * (size_t)p.ldc * 2, m < p.M, lane);
+        for (int pass = 0; pass < passes; ++pass) {
+          const bool do_act = p.act == ACT_GELU && (!p.dual_out || pass == 1);
+#pragma unroll 1
+          for (int c = c_lo; c < c_hi; ++c) {
+            uint32_t v[32];
+            tmem_ld32(tacc + 32 * c, v);
+            tmem_wait_ld();
+            uint4 u[4];
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+              float f[8];
+#pragma unroll
+              for (int e = 0; e < 8; ++e) f[e] = has_k ? __uint_as_float(v[8 * ch + e]) * rs : 0.f;
+              if (do_act) {
+#pragma unroll
+                for (int e = 0; e < 8; e += 2) gelu_pair(f[e], f[e + 1]);
+              }
+              u[ch] = pack8(f);
+            }
+            const int col = n0 + 32 * c;
+            int t = p.split_cols > 0 ? col / p.split_cols : 0;
+            const int cin = col - t * p.split_cols;
+            if (p.dual_out) t = pass;
+            unsigned char* base = p.c_ptr[t] + ((size_t)bz * (size_t)p.c_bstride + (size_t)cin) * 2;
+            quad_transpose(u, lane);
+            const bool col_ok = col + 8 * (lane & 3) < p.N;
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4)
+              if (qr.live[k4] && col_ok) stg_v4(base + qr.off[k4], u[k4]);
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&bar_acc_free[ab]));
+        if (traced && threadIdx.x == 64) TR(5, it);           // tile stored
+      }
+      continue;
+    }
     // the staging tile: free once the previous tile's store has read it (with an auxiliary tile the producer waited
     // for that before loading it)
     if (p.aux_mode != AUX_NONE) mbar_wait(smem_u32(&bar_aux), it & 1);
@@ -433,10 +488,12 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   if (!ok) return cudaErrorInvalidValue;
   auto kern = gemm_tc_kernel<BN, A_MN, B_MN>;
   static SmemAttr attr;
-  cudaError_t e = attr.ensure(kern, BN > 128 ? Cfg<BN>::SMEM_SPLITK : Cfg<BN>::SMEM_AUX, di->ordinal);
+  constexpr int kSmemMax = BN > 128 ? Cfg<BN>::SMEM_SPLITK
+                                    : (Cfg<BN>::SMEM_AUX > Cfg<BN>::SMEM_DIRECT ? Cfg<BN>::SMEM_AUX : Cfg<BN>::SMEM_DIRECT);
+  cudaError_t e = attr.ensure(kern, kSmemMax, di->ordinal);
   if (e != cudaSuccess) return e;
   if (BN > 128 && !p.partial) return cudaErrorInvalidValue;   // (256-wide tiles: split-K only)
-  const int smem = p.partial ? Cfg<BN>::SMEM_SPLITK : Cfg<BN>::SMEM_AUX;
+  const int smem = p.partial ? Cfg<BN>::SMEM_SPLITK : (p.aux_mode == AUX_NONE ? Cfg<BN>::SMEM_DIRECT : Cfg<BN>::SMEM_AUX);
   // row tiles per launch: all of them (split-K, batched and small problems), else as many as keep every CTA resident
   // (three per SM); each CTA then walks its column of row tiles (see the kernel)
   const int tiles_n = (p.N + BN - 1) / BN, tiles_m = (p.M + BM - 1) / BM, gz = p.partial ? kp.slabs : p.batch;
@@ -496,6 +553,8 @@ cudaError_t launch(const Problem& p, cudaStream_t stream) {
   kp.partial = p.partial; kp.split_cols = p.split_cols;
   kp.a_batched = p.A.batch_stride != 0; kp.b_batched = p.B.batch_stride != 0;
   kp.a_split_k = p.a_split_k; kp.a_split_m = p.a_split_m; kp.dual_out = p.dual_out;
+  for (int t = 0; t < 3; ++t) kp.c_ptr[t] = static_cast<unsigned char*>(p.C[t] ? p.C[t] : p.C[0]);
+  kp.ldc = p.ldc; kp.c_bstride = p.c_batch_stride;
   if (p.a_split_m > 0 && (p.a_split_m % 128 != 0 || p.M != 3 * p.a_split_m || !p.A2 || !p.A3 || !p.A.mn_major || p.a_split_k > 0))
     return cudaErrorInvalidValue;
   if (p.a_split_k > 0 && (p.a_split_k % 64 != 0 || p.K != 3 * p.a_split_k || !p.A2 || !p.A3)) return cudaErrorInvalidValue;
