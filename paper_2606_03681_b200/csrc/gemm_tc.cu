@@ -1,9 +1,11 @@
 // tcgen05 GEMM core (gemm_tc.cuh): 128 x BN output tiles, a 2-3 stage TMA ring over 64-wide k-blocks, fp32 accumulators
 // in TMEM, fused epilogue, TMA store.  Warp 0 = TMA producer (one lane), warp 1 = MMA issuer (owns the TMEM
 // allocation), warps 2-9 = epilogue (one thread per accumulator row and column half).  A CTA is persistent over the
-// row tiles of its column tile and alternates TWO accumulators, so that tile i's epilogue (TMEM -> registers -> staging
-// tile -> TMA store) runs under tile i+1's loads and MMAs; two such CTAs fit an SM (96 KB of shared memory and 256
-// TMEM columns each at BN = 128).  These contractions have K = 192..768 only: a tile is 4-12 k-blocks of work and the
+// row tiles of its column tile and alternates TWO accumulators, so that tile i's epilogue runs under tile i+1's loads
+// and MMAs; two such CTAs fit an SM (96 KB of shared memory and 256 TMEM columns each at BN = 128).  Two epilogues:
+// with an auxiliary tile (residual, gelu') the tile is prefetched by TMA into a staging tile, overwritten in place and
+// stored by TMA, behind a two-stage ring; without one the epilogue stores straight from registers (quad-transposed
+// rows) and the staging tile's shared memory is a third ring stage.  These contractions have K = 192..768 only: a tile is 4-12 k-blocks of work and the
 // kernels are bound by HBM and the epilogue, not by the tensor pipe (profiles/r02_blocks.md).
 #include "gemm_tc.cuh"
 
