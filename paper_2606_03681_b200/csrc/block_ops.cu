@@ -8,6 +8,8 @@
 #include "common.cuh"
 #include "device.h"
 #include "gemm_tc.cuh"
+#include <algorithm>
+
 #include "kernels.h"
 
 namespace tabattn {
@@ -279,9 +281,18 @@ cudaError_t weight_grad(const void* dY, long long ldy, const void* A, long long 
   if (dY2) { p.A2 = dY2; p.A3 = dY3; p.a_split_m = N / 3; }
   p.B = {A, 1, lda, 0};
   p.alpha = 1.f;
-  // (column tiles: 256 wide when K allows it, else 128 / 64 -- gemm::launch)
-  const int tiles = ((N + 127) / 128) * (K % 256 == 0 ? K / 256 : (K + 63) / 64);
-  p.slabs = gemm::slabs_for(M, tiles, di->num_sms);
+  // (256 x 256 tiles when K allows it, else 128 x 128 / 64 -- gemm::launch)
+  const int tiles = K % 256 == 0 ? ((N + 255) / 256) * (K / 256) : ((N + 127) / 128) * ((K + 63) / 64);
+  if (K % 256 == 0) {
+    // one 256 x 256 CTA per SM (192 KB of ring): as many slabs as give one wave
+    const long long kb_total = (M + 63) / 64;
+    long long want = std::max(1, std::min(128, di->num_sms / tiles));
+    if (want > kb_total) want = kb_total;
+    const long long per = (kb_total + want - 1) / want;
+    p.slabs = (int)((kb_total + per - 1) / per);
+  } else {
+    p.slabs = gemm::slabs_for(M, tiles, di->num_sms);
+  }
   if ((size_t)p.slabs * N * K > ws_floats) return cudaErrorInvalidValue;
   p.partial = ws_f32;
   cudaError_t e = gemm::launch(p, stream);

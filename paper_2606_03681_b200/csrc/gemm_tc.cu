@@ -101,13 +101,17 @@ __device__ __forceinline__ void gelu_grad_pair(float x0, float x1, float& g0, fl
 
 template <int BN>
 struct Cfg {
-  static constexpr int ST = BN == 64 ? 3 : 2;
+  // BN = 256 (split-K weight gradients only): a CTA computes TWO row tiles, 256 x 256, from one B stage -- these
+  // kernels are bound by operand traffic from L2 (~8.5 TB/s) and this fetches every operand byte the fewest times
+  static constexpr bool PAIR = BN == 256;
+  static constexpr int A_STAGE = (PAIR ? 2 : 1) * A_BYTES;
+  static constexpr int ST = BN == 128 ? 2 : 3;
   // ring depth when the epilogue needs no staging tile (it stores straight from registers): the freed shared memory
   // holds one more stage -- the plain projections are bound by the latency of their operand loads (timeline,
   // profiles/r02_blocks.md: a round trip is ~2,400 clk and a K = 768 tile was six of them)
   static constexpr int ST_DIRECT = ST + 1, ST_MAX = ST_DIRECT;
   static constexpr int B_BYTES = BN * BK * 2;
-  static constexpr int STAGE = A_BYTES + B_BYTES;
+  static constexpr int STAGE = A_STAGE + B_BYTES;
   static constexpr int STAGING = (BN / 64) * (BM * 128);
   // the epilogue's staging tile is a buffer of its own (an auxiliary tile is prefetched into it when there is one):
   // the ring keeps loading the next tile while the epilogue of the current one writes it
@@ -132,7 +136,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const bool direct = BN <= 128 && p.aux_mode == AUX_NONE && p.partial == nullptr;
   const uint32_t st_n = direct ? C::ST_DIRECT : ST;          // ring depth
-  const uint32_t sA = sbase, sB = sA + st_n * A_BYTES;
+  const uint32_t sA = sbase, sB = sA + st_n * C::A_STAGE;
   const uint32_t sOut = sB + st_n * C::B_BYTES;   // the epilogue's staging tile (the auxiliary tile lands in it first)
   __shared__ uint64_t bar_full[C::ST_MAX], bar_empty[C::ST_MAX], bar_acc[2], bar_aux, bar_acc_free[2], bar_out_free;
   __shared__ uint32_t tmem_slot;
@@ -141,7 +145,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   // A CTA walks the row tiles my = blockIdx.y, blockIdx.y + gridDim.y, ... of its column tile (the host sizes
   // gridDim.y so that all CTAs are resident at once): TMEM allocation, barrier set-up and the CTA launch are paid once
   // per CTA instead of once per 128 x BN tile -- with K = 256..768 a tile is only 4-12 k-blocks of work.
-  const int n0 = blockIdx.x * BN, tiles_m = (p.M + BM - 1) / BM;
+  constexpr int BMT = C::PAIR ? 2 * BM : BM;   // rows per CTA step
+  const int n0 = blockIdx.x * BN, tiles_m = (p.M + BMT - 1) / BMT;
   const bool splitk = p.partial != nullptr;   // fp32 partial tiles instead of the bf16 output
   const int bz = splitk ? 0 : blockIdx.z, slab = splitk ? blockIdx.z : 0;
   const int kb0 = slab * p.kb_per_slab, kb1 = min(p.kb_total, kb0 + p.kb_per_slab);
@@ -152,7 +157,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   // touches global memory before the predecessor has completed and flushed.  (Chains of small GEMMs -- the 16
   // launches of Newton-Schulz -- are latency-bound: ~7 us per kernel.)
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), splitk ? BN : 2 * BN);
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_slot), (splitk && !C::PAIR) ? BN : 2 * BN);
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::ST_MAX; ++i) {
       mbar_init(smem_u32(&bar_full[i]), 1);
@@ -179,7 +184,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       const int ba = p.a_batched ? bz : 0, bb = p.b_batched ? bz : 0;
       uint32_t st = 0, ph = 0, it = 0;
       for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
-      const int m0 = my * BM;
+      const int m0 = my * BMT;
       // (the A / B loads of a tile run ahead under the previous tile's epilogue; the auxiliary load, below, waits for
       // the staging tile)
       for (int kb = kb0; kb < kb1; ++kb) {
@@ -187,17 +192,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         mbar_wait<true>(smem_u32(&bar_empty[st]), ph ^ 1);
         if (traced && kb == kb0) TR(0, it);                 // first stage of the tile free, loads start
         mbar_arrive_expect_tx(full, C::STAGE);
-        const uint32_t a = sA + st * A_BYTES, b = sB + st * C::B_BYTES;
+        const uint32_t a = sA + st * C::A_STAGE, b = sB + st * C::B_BYTES;
         if (A_MN) {
-          const CUtensorMap* ma = &mapA;
-          int ml = m0;
-          if (p.a_split_m > 0) {
-            const int seg = m0 / p.a_split_m;
-            ml = m0 - seg * p.a_split_m;
-            ma = seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3);
+#pragma unroll
+          for (int mt = 0; mt < (C::PAIR ? 2 : 1); ++mt) {
+            const CUtensorMap* ma = &mapA;
+            int ml = m0 + BM * mt;
+            if (p.a_split_m > 0) {
+              const int seg = min(ml / p.a_split_m, 2);
+              ml -= seg * p.a_split_m;
+              ma = seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3);
+            }
+            tma_load_3d(a + mt * A_BYTES, ma, full, ml, kb * BK, ba);
+            tma_load_3d(a + mt * A_BYTES + 64 * 128, ma, full, ml + 64, kb * BK, ba);
           }
-          tma_load_3d(a, ma, full, ml, kb * BK, ba);
-          tma_load_3d(a + 64 * 128, ma, full, ml + 64, kb * BK, ba);
         } else if (p.a_split_k > 0) {
           const int seg = (kb * BK) / p.a_split_k, kin = kb * BK - seg * p.a_split_k;
           tma_load_3d(a, seg == 0 ? &mapA : (seg == 1 ? &mapA2 : &mapA3), full, kin, m0, ba);
@@ -239,11 +247,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         mbar_wait(smem_u32(&bar_full[st]), ph);
         if (traced && lane == 0 && kb == kb0) TR(2, it);    // first k-block landed
         tc_fence_after();
-        const uint64_t a = dA + (uint64_t)((st * A_BYTES) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
+        const uint64_t a = dA + (uint64_t)((st * C::A_STAGE) >> 4), b = dB + (uint64_t)((st * C::B_BYTES) >> 4);
 #pragma unroll
-        for (int kk = 0; kk < BK / 16; ++kk)
+        for (int kk = 0; kk < BK / 16; ++kk) {
           mma_ss_e(acc, a + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc,
                    (kb > kb0 || kk > 0) ? 1u : 0u);
+          if constexpr (C::PAIR)   // the second row tile of the pair, same B stage, second accumulator
+            mma_ss_e(acc + BN, a + (A_BYTES >> 4) + (A_MN ? kk * 128 : 2 * kk), b + (B_MN ? kk * 128 : 2 * kk), idesc,
+                     (kb > kb0 || kk > 0) ? 1u : 0u);
+        }
         tc_commit_e(smem_u32(&bar_empty[st]));
         if (++st == st_n) { st = 0; ph ^= 1; }
       }
@@ -259,7 +271,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     const int passes = p.dual_out ? 2 : 1;
     uint32_t it = 0;
     for (int my = blockIdx.y; my < tiles_m; my += gridDim.y, ++it) {
-    const int m0 = my * BM, m = m0 + r;
+    const int m0 = my * BMT, m = m0 + r;
     float rs = p.alpha;
     if (p.row_scale && m < p.M) rs *= __ldg(p.row_scale + (size_t)bz * p.M + m);
     const uint32_t ab = it & 1, tacc = tacc0 + ab * BN;
@@ -327,14 +339,26 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
           for (int j = 0; j < 32; ++j) v[j] = 0u;
         }
         if (splitk) {
-          if (m < p.M) {
-            float* dst = p.partial + ((size_t)slab * p.M + m) * p.N + n0 + 32 * c;
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-              if (n0 + 32 * c + 4 * j < p.N)
-                *reinterpret_cast<float4*>(dst + 4 * j) =
-                    make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
-                                __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+          for (int mt = 0; mt < (C::PAIR ? 2 : 1); ++mt) {
+            if (mt == 1) {   // the pair's second row tile (second accumulator)
+              tmem_ld32(tacc + BN + 32 * c, v);
+              tmem_wait_ld();
+              if (!has_k) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) v[j] = 0u;
+              }
+            }
+            const int mm = m + BM * mt;
+            if (mm < p.M) {
+              float* dst = p.partial + ((size_t)slab * p.M + mm) * p.N + n0 + 32 * c;
+#pragma unroll
+              for (int j = 0; j < 8; ++j)
+                if (n0 + 32 * c + 4 * j < p.N)
+                  *reinterpret_cast<float4*>(dst + 4 * j) =
+                      make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                  __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+            }
           }
           continue;
         }
@@ -408,7 +432,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, splitk ? BN : 2 * BN);
+  if (warp == 1) tmem_dealloc(tmem, (splitk && !C::PAIR) ? BN : 2 * BN);
 }
 
 __global__ void reduce_slabs_kernel(const float* __restrict__ partial, int slabs, long long mn, float scale,
@@ -498,7 +522,8 @@ cudaError_t launch_t(const Problem& p, const KParams& kp, cudaStream_t stream) {
   const int smem = p.partial ? Cfg<BN>::SMEM_SPLITK : (p.aux_mode == AUX_NONE ? Cfg<BN>::SMEM_DIRECT : Cfg<BN>::SMEM_AUX);
   // row tiles per launch: all of them (split-K, batched and small problems), else as many as keep every CTA resident
   // (three per SM); each CTA then walks its column of row tiles (see the kernel)
-  const int tiles_n = (p.N + BN - 1) / BN, tiles_m = (p.M + BM - 1) / BM, gz = p.partial ? kp.slabs : p.batch;
+  constexpr int kRowsPerCta = BN == 256 ? 2 * BM : BM;   // (256-wide tiles come in pairs of row tiles)
+  const int tiles_n = (p.N + BN - 1) / BN, tiles_m = (p.M + kRowsPerCta - 1) / kRowsPerCta, gz = p.partial ? kp.slabs : p.batch;
   int gy = tiles_m;
   if (!p.partial) gy = std::min(tiles_m, std::max(1, (2 * di->num_sms) / (tiles_n * gz)));
   dim3 grid(tiles_n, gy, gz);
