@@ -54,3 +54,43 @@ def test_graph_replay_equals_direct_calls(cfg):
         for i, (a, b) in enumerate(zip(_results(g_buf), _results(ref_buf))):
             assert torch.isfinite(b.float()).all(), "direct result %d not finite" % i
             assert _same(a, b), "round %d: result %d differs between graph replay and direct calls" % (round_, i)
+
+
+def test_mlp_block_and_newton_schulz_replay_equal_direct_calls():
+    """The GEMM kernels are launched with programmatic dependent launch; a captured chain of them (MLP sub-block forward
+    and backward, Newton-Schulz) must replay to the bits of the direct calls."""
+    import paper_2606_03681_b200 as tab
+    dev = torch.device("cuda", 0)
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    cells, e, hid = 1500, 256, 768
+    bf = torch.bfloat16
+    x = torch.randn((cells, e), generator=g, device=dev).to(bf)
+    dy = torch.randn((cells, e), generator=g, device=dev).to(bf)
+    gain = (1.0 + 0.1 * torch.randn((e,), generator=g, device=dev)).to(bf)
+    w1 = (torch.randn((hid, e), generator=g, device=dev) * e ** -0.5).to(bf)
+    w2 = (torch.randn((e, hid), generator=g, device=dev) * hid ** -0.5).to(bf)
+    G = (torch.randn((6, 128, 256), generator=g, device=dev) * 0.02).to(bf)
+
+    def run():
+        y, saved = tab.tabattn_mlp_fwd(x, gain, w1, w2, 0.9)
+        grads = tab.tabattn_mlp_bwd(x, gain, w1, w2, saved, dy, 0.9)
+        X = tab.tabattn_newton_schulz(G, 5)
+        return (y,) + tuple(grads) + (X,)
+
+    want = run()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            got = run()
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(2):
+        for t in got:
+            t.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for i, (a, b) in enumerate(zip(got, want)):
+            assert _same(a, b), "result %d differs between graph replay and direct calls" % i
