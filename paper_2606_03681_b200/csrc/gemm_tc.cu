@@ -130,8 +130,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   TR_INIT();
   using C = Cfg<BN>;
   constexpr int ST = C::ST;
-  // (trace builds: only the projections with split or dual outputs -- the QKV and the MLP up-projection -- are stamped)
-  [[maybe_unused]] const bool traced = p.split_cols > 0 || p.dual_out;
+  // (trace builds: only the QKV projection, the MLP up-projection and the gelu' product are stamped)
+  [[maybe_unused]] const bool traced = p.split_cols > 0 || p.dual_out || p.aux_mode == AUX_GELU_GRAD;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const bool direct = BN <= 128 && p.aux_mode == AUX_NONE && p.partial == nullptr;

@@ -1,11 +1,12 @@
 """Timeline of the GEMM core on one CTA (developer tool; needs a B200 and a trace build).
 
     TABATTN_TRACE=1 python -m paper_2606_03681_b200.build --force
-    python -m paper_2606_03681_b200.trace_gemm [qkv|up]
+    python -m paper_2606_03681_b200.trace_gemm [qkv|up|gg]
     python -m paper_2606_03681_b200.build --force          # back to the shipped library
 
 `qkv`: the QKV projection of the attention sub-block (688,128 cells, e = 256: K = 256, N = 768 into three tensors);
-`up`: the MLP up-projection (K = 256, N = 768, two outputs).  Prints, for row tiles 2..41 of CTA 0, the clock64() stamps
+`up`: the MLP up-projection (K = 256, N = 768, two outputs); `gg`: du = (dy W2) o gelu'(u) of the MLP backward
+(K = 256, N = 768, auxiliary tile u).  Prints, for row tiles 2..41 of CTA 0, the clock64() stamps
 (relative to the first) of the events named in csrc/gemm_tc.cu (TR(...)): producer (loads start, last load issued), MMA
 warp (first k-block landed, MMAs issued), first epilogue warp (accumulator complete, its staging part written, all
 warps done, store issued, staging read; a second group of four for the second output of `up`), and the tile-to-tile
@@ -41,7 +42,12 @@ def main():
     else:
         w1 = (torch.randn((hid, e), generator=g, device=dev) * e ** -0.5).to(bf)
         w2 = (torch.randn((e, hid), generator=g, device=dev) * hid ** -0.5).to(bf)
-        run = lambda: tab.tabattn_mlp_fwd(x.view(cells, e), gain, w1, w2, 1.0)
+        if which == "up":
+            run = lambda: tab.tabattn_mlp_fwd(x.view(cells, e), gain, w1, w2, 1.0)
+        else:
+            _, saved = tab.tabattn_mlp_fwd(x.view(cells, e), gain, w1, w2, 1.0)
+            dy = torch.randn((cells, e), generator=g, device=dev, dtype=torch.float32).to(bf)
+            run = lambda: tab.tabattn_mlp_bwd(x.view(cells, e), gain, w1, w2, saved, dy, 1.0)
     for _ in range(3):
         run()
     trace = torch.zeros(64 * 16, dtype=torch.int64, device=dev)
