@@ -37,10 +37,11 @@ MLP_CASES = [
     (300, 64, 128, 1.0),          # ragged last tile (300 = 2 * 128 + 44)
     (1000, 192, 768, 0.95 ** 2),  # the baseline width
     (777, 256, 768, 1.0),         # the record width
+    (20000, 256, 768, 1.0),       # 157 row tiles: every persistent GEMM CTA walks several (148 CTAs per column tile)
 ]
 
 
-@pytest.mark.parametrize("case", MLP_CASES, ids=["e64", "e192", "e256"])
+@pytest.mark.parametrize("case", MLP_CASES, ids=["e64", "e192", "e256", "e256_multi_tile"])
 def test_mlp_block_parity(case):
     import torch
     import paper_2606_03681_b200 as tab
